@@ -1,0 +1,313 @@
+#!/usr/bin/env python3
+"""bench.py -- throughput of the hot path on the workload BASELINE.json's metric is quoted on.
+
+Workload (BASELINE.json configs[1], "C2"): Henon-Heiles arc-length Lagrangian descriptor,
+E = 1/8, 1024 x 1024 energy-fitted grid of (y, py) on the x = 0 section, forward and backward
+fixed-step DOP8, h = 0.01, |t| = 50 (5000 steps per direction), FP64.  One "step" of this
+benchmark = one pass of the whole hot path over that batch = 2 * 1048576 * 5000 RK-steps,
+one kernel launch.  Metric: trajectory RK-steps/sec.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C2|C1sat]
+
+N > 1 (torchrun): every rank integrates its own 1024 x 1024 block of rows of a (1024 N) x 1024
+grid (weak scaling, no data-path collective: trajectories are independent).
+`--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload.
+Prints ONE JSON line on rank 0.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "trajectory RK-steps/sec (FP64, incl. variational eqs)"
+UNIT = "RK-steps/s"
+# algorithmic FP64 flop per RK-step of the formulation that runs
+FLOP_PER_STEP = {"C2": 640.0, "C1sat": 1128.0}
+NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12  # 37.2
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C2", choices=["C2", "C1sat"])
+    ap.add_argument("--side", type=int, default=1024, help="grid side per rank (C2)")
+    ap.add_argument("--n-steps", type=int, default=5000, help="DOP8 steps per direction (C2)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.stop, self.th = index, [], threading.Event(), None
+
+    def _run(self):
+        while not self.stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5)
+                self.rows.append([x.strip() for x in out.stdout.strip().split(",")])
+            except Exception:
+                pass
+            self.stop.wait(0.2)
+
+    def __enter__(self):
+        self.th = threading.Thread(target=self._run, daemon=True)
+        self.th.start()
+        return self
+
+    def __exit__(self, *a):
+        self.stop.set()
+        self.th.join(timeout=6)
+
+    def summary(self):
+        sm, mx, reasons = [], 0, set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx = max(mx, float(r[1]))
+                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+            except Exception:
+                pass
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx or None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def workload_inputs(args, rank, world):
+    from paper_2507_00622_b200 import workloads as W
+    if args.workload == "C2":
+        side = args.side
+        y0 = W.hh_grid(0.125, side * world, side, i_range=(rank * side, (rank + 1) * side))
+        return dict(y0=y0, h=0.01, n_steps=args.n_steps, rk_steps=2.0 * y0.shape[1] * args.n_steps)
+    # C1sat: the fixed-step SALI kernel of configs[0] on a saturating ensemble
+    side = 512
+    y0 = W.hh_grid(0.125, side * world, side, i_range=(rank * side, (rank + 1) * side))
+    w0 = W.deviation_vectors(y0.shape[1], 2, 4, 0, "unit")
+    return dict(y0=y0, w0=w0, h=0.01, n_steps=2000, rk_steps=1.0 * y0.shape[1] * 2000)
+
+
+def run_reference(args):
+    """The CPU oracle, as it stands, on a bounded sample of the same workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import chaos_oracle as orc
+    from paper_2507_00622_b200 import workloads as W
+    orc.build()
+    cores = orc.default_threads()
+    sub = 48  # 48 x 48 sub-grid of the 1024 x 1024 grid (every ~21st row / column), full horizon
+    idx = (np.arange(sub) * (args.side // sub))
+    full_rows = [W.hh_grid(0.125, args.side, args.side, i_range=(int(i), int(i) + 1))[:, idx] for i in idx]
+    y0 = np.ascontiguousarray(np.concatenate(full_rows, axis=1))
+    n_steps = args.n_steps
+    times = []
+    for it in range(args.warmup + args.steps):
+        t = time.perf_counter()
+        orc.ld(0, None, y0, 0.0, 0.01, n_steps, precision="f64", threads=cores)
+        dt = time.perf_counter() - t
+        if it >= args.warmup:
+            times.append(dt)
+    rk = 2.0 * y0.shape[1] * n_steps
+    val = rk * len(times) / sum(times)
+    sample = f"{sub}x{sub} sub-grid of the {args.side}x{args.side} grid, full horizon ({n_steps} steps x 2 directions)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sum(times) / len(times),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "C2: Henon-Heiles LD, E=1/8, fixed DOP8 h=0.01, fwd+bwd (CPU oracle on a bounded sample)",
+                   "n_ic_sample": int(y0.shape[1]), "n_steps_per_direction": n_steps},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2507_00622_b200 import binding as chs  # raises if the library is missing
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    wl = workload_inputs(args, rank, world)
+    y0_host = torch.from_numpy(wl["y0"]).pin_memory()
+    y0 = y0_host.cuda()
+    n_ic = y0.shape[1]
+    HH = chs.SYS_HENON_HEILES
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
+
+    if args.workload == "C2":
+        f = torch.empty(n_ic, dtype=torch.float64, device="cuda")
+        b = torch.empty(n_ic, dtype=torch.float64, device="cuda")
+        f_host = torch.empty(n_ic, dtype=torch.float64).pin_memory()
+        b_host = torch.empty(n_ic, dtype=torch.float64).pin_memory()
+
+        def step_dev():
+            chs.ld(HH, None, y0, 0.0, wl["h"], wl["n_steps"], out_fwd=f, out_bwd=b)
+
+        def step_e2e():
+            chs.ld_host(HH, None, y0_host, 0.0, wl["h"], wl["n_steps"], f_host, b_host)
+
+        h2d, d2h = y0_host.numel() * 8, 2 * n_ic * 8
+        kinfo = chs.kernel_info(HH, None, chs.WHAT_LD, n_ic=n_ic)
+        launches_per_step = 1
+    else:
+        w0_host = torch.from_numpy(wl["w0"]).pin_memory()
+        w0 = w0_host.cuda()
+        yb, wb = torch.empty_like(y0), torch.empty_like(w0)
+        yh, wh = torch.empty_like(y0_host).pin_memory(), torch.empty_like(w0_host).pin_memory()
+        sh = torch.empty((1, n_ic), dtype=torch.float64).pin_memory()
+
+        def step_dev():
+            yb.copy_(y0)
+            wb.copy_(w0)
+            chs.sali(HH, None, yb, wb, renorm_every=1, h=wl["h"], n_steps=wl["n_steps"])
+
+        def step_e2e():
+            yh.copy_(y0_host)
+            wh.copy_(w0_host)
+            chs.sali_host(HH, None, yh, wh, sh, renorm_every=1, h=wl["h"], n_steps=wl["n_steps"])
+
+        h2d, d2h = (y0_host.numel() + w0_host.numel()) * 8, (y0_host.numel() + w0_host.numel() + n_ic) * 8
+        kinfo = chs.kernel_info(HH, None, chs.WHAT_SALI, k=2, n_ic=n_ic)
+        launches_per_step = 1
+
+    def timed(fn, n):
+        """n iterations, each bracketed by CUDA events on the launching stream, L2 flushed between."""
+        ms = []
+        for _ in range(n):
+            flush.fill_(1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            fn()
+            e1.record()
+            torch.cuda.synchronize()
+            ms.append(e0.elapsed_time(e1))
+        return ms
+
+    # FP64 FMA peak of this device, measured live (register-only DFMA chains)
+    chs.dfma_probe(1000, 148 * 8)
+    torch.cuda.synchronize()
+    pe0, pe1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    pe0.record()
+    probe_flop, _ = chs.dfma_probe(400000, 148 * 8)
+    pe1.record()
+    torch.cuda.synchronize()
+    dfma_tflops = probe_flop / (pe0.elapsed_time(pe1) * 1e-3) / 1e12
+
+    for _ in range(max(args.warmup, 0)):
+        step_dev()
+    barrier()
+    with ClockSampler(local) as cs:
+        t_wall = time.perf_counter()
+        ms = timed(step_dev, args.steps)
+        barrier()
+        t_wall = time.perf_counter() - t_wall
+    clocks = cs.summary()
+    t_dev = sum(ms) * 1e-3
+    if world > 1:
+        tt = torch.tensor([t_dev], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_dev = tt.item()
+    value = wl["rk_steps"] * world * args.steps / t_dev
+
+    # end to end: host buffers through the C ABI's host entry point, copies inside the timed region
+    step_e2e()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step_e2e()
+    torch.cuda.synchronize()
+    t_e2e = time.perf_counter() - t0
+    if world > 1:
+        tt = torch.tensor([t_e2e], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_e2e = tt.item()
+    e2e_value = wl["rk_steps"] * world * args.steps / t_e2e
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    flop = FLOP_PER_STEP[args.workload]
+    achieved = flop * wl["rk_steps"] / (np.mean(ms) * 1e-3) / 1e12
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * t_dev / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {
+            "workload": ("C2: Henon-Heiles Lagrangian descriptor (arc length), E=1/8, %dx%d grid per GPU, "
+                         "fixed DOP8 h=0.01, %d steps forward + %d backward" % (args.side, args.side, wl["n_steps"], wl["n_steps"]))
+            if args.workload == "C2" else
+            "C1sat: Henon-Heiles fixed-step SALI kernel of configs[0] on a saturating 512x512 ensemble, 2000 steps",
+            "n_ic_per_gpu": int(n_ic), "rk_steps_per_step": wl["rk_steps"] * world,
+            "l2": "flushed between timed iterations (256 MiB write)",
+            "kernel": kinfo,
+        },
+        "roofline": {
+            "bound": "alu", "achieved": achieved, "peak": NOMINAL_FP64_TFLOPS, "unit": "TFLOP/s",
+            "frac": achieved / NOMINAL_FP64_TFLOPS, "traffic": None,
+            "peak_source": "nominal: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz (DESIGN.md Roofline)",
+            "measured_dfma_tflops": dfma_tflops, "frac_of_measured_dfma": achieved / dfma_tflops,
+            "flop_per_rk_step": flop, "kernel_ms": float(np.mean(ms)),
+        },
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
+        "gpu_launches": launches_per_step * args.steps,
+        "clocks": clocks,
+        "wall_s_timed_region": t_wall,
+    }
+    if not args.no_cpu_baseline and world == 1 and args.workload == "C2":
+        from oracle import chaos_oracle as orc
+        orc.build()
+        cores = orc.default_threads()
+        sub = 48
+        idx = np.arange(sub) * (args.side // sub)
+        ys = np.ascontiguousarray(wl["y0"].reshape(4, args.side, args.side)[:, idx][:, :, idx].reshape(4, -1))
+        t0 = time.perf_counter()
+        orc.ld(0, None, ys, 0.0, 0.01, wl["n_steps"], precision="f64", threads=cores)
+        dt = time.perf_counter() - t0
+        out["cpu_baseline"] = {
+            "value": 2.0 * ys.shape[1] * wl["n_steps"] / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{sub}x{sub} sub-grid of the same grid, full horizon, {dt:.1f} s"}
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

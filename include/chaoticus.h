@@ -1,0 +1,163 @@
+/* chaoticus.h -- C ABI of the B200-native (sm_100a, FP64) ensemble integrator.
+ *
+ * The hot path of arXiv 2507.00622 ("Chaoticus", /root/reference/PAPER.md): huge ensembles of
+ * independent initial conditions of a Hamiltonian system integrated with the
+ * 8th-order Dormand-Prince method, fixed step "DOP 8" or adaptive "DOP 8(5)" (PAPER.md:43,
+ * PAPER.md:47-53), each trajectory carrying its variational equations and
+ * accumulating a chaos indicator as it goes: SALI, GALI_k from singular values
+ * (PAPER.md:55), the arc-length Lagrangian descriptor, or the
+ * Lyapunov spectrum via QR / Gram-Schmidt.
+ *
+ * CONVENTIONS (every entry point)
+ *  - Pointers marked DEVICE are CUDA device pointers to FP64 (or the stated integer type) in
+ *    the current device's memory; pointers marked HOST are ordinary host pointers.
+ *  - Layout is structure-of-arrays, component-major / IC-minor:
+ *        y[c * n_ic + ic],            c < n            (n = phase-space dimension 2N,
+ *        w[(v * n + c) * n_ic + ic],  v < k                 ordering (q_1..q_N, p_1..p_N))
+ *        out[s * n_ic + ic]           for per-sample / per-vector outputs.
+ *  - Ownership: the caller owns every buffer.  Device-pointer entry points allocate nothing,
+ *    free nothing, and only ENQUEUE work on `stream` (a cudaStream_t passed as void*; NULL =
+ *    the legacy default stream); they do not synchronise.  The *_host entry points allocate
+ *    their own device scratch, copy in, run, copy out, synchronise and free before returning.
+ *  - y and w are advanced IN PLACE to the final time, w is returned normalised
+ *    (orthonormalised by chaoticus_lyap), so a second call continues the run.
+ *  - Errors: argument errors return CHS_EINVAL (nothing is launched); a system / k / size
+ *    with no compiled kernel returns CHS_EUNSUPPORTED; a CUDA failure returns CHS_ECUDA.
+ *    chaoticus_last_error() gives a message.  Trouble of ONE trajectory is not a call error:
+ *    it sets status[ic] (CHS_ST_*) and that trajectory's y, w and outputs are NaN.
+ *  - n_ic = 0 is a valid no-op.  There is no CPU fallback: without a CUDA device every
+ *    compute entry point returns CHS_ECUDA.
+ */
+#ifndef CHAOTICUS_H
+#define CHAOTICUS_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CHAOTICUS_VERSION 100 /* 0.1.0 */
+
+typedef enum { CHS_OK = 0, CHS_EINVAL = 1, CHS_EUNSUPPORTED = 2, CHS_ECUDA = 3 } chs_rc;
+
+/* Systems (all separable, H = |p|^2/2 + V(q)):
+ *  CHS_SYS_HENON_HEILES  n = 4, no params.  PAPER.md:87 Eq.(4), Eq.(5).
+ *  CHS_SYS_COUPLED3      n = 6, params (omega1, omega2, omega3, eps):
+ *                        V = sum omega_i^2 q_i^2 / 2 + eps q1^2 q2 + eps q2^2 q3
+ *                        (BASELINE.json configs[3]; eps = 0: uncoupled oscillators).
+ *  CHS_SYS_FPUT          n = 2N, params (N, k, alpha, beta), N given as a double, fixed ends
+ *                        q_0 = q_{N+1} = 0, N+1 springs.  PAPER.md:98 Eq.(6),
+ *                        PAPER.md:103-106 Eq.(7), Eq.(8).  Compiled N: 2,4,8,16,32. */
+typedef enum { CHS_SYS_HENON_HEILES = 0, CHS_SYS_COUPLED3 = 1, CHS_SYS_FPUT = 2 } chs_system;
+
+typedef struct {
+    int system;           /* chs_system */
+    int n_params;         /* number of doubles at params */
+    const double* params; /* HOST; read during the call only */
+} chs_problem;
+
+/* Stepper.  adaptive = 0: n_steps steps of signed size h from t0 ("DOP 8").
+ * adaptive = 1: from t0 to t_end with per-trajectory step control ("DOP 8(5)", PAPER.md:48,
+ * error estimate PAPER.md:53): err = |h| S5 / sqrt(D (S5 + 0.01 S3)) over all D components of
+ * the augmented state, scale = atol + rtol max(|y|,|y+|); accept iff err < 1; step factor
+ * 0.9 err^(-1/8) clipped to [0.2, 10] (<= 1 after a rejection); last step lands on t_end;
+ * h0 <= 0 selects the automatic starting step; max_steps <= 0 = unbounded attempts. */
+typedef struct {
+    int adaptive;
+    double t0;
+    double h;            /* fixed */
+    long long n_steps;   /* fixed */
+    double t_end, rtol, atol, h0; /* adaptive */
+    long long max_steps;          /* adaptive */
+} chs_stepper;
+
+/* Per-trajectory report; every member is DEVICE [n_ic] or NULL. */
+#define CHS_ST_OK 0
+#define CHS_ST_NONFINITE 1
+#define CHS_ST_UNDERFLOW 2
+#define CHS_ST_MAXSTEPS 3
+typedef struct {
+    long long* n_accepted; /* accepted steps (fixed: n_steps) */
+    long long* n_rejected; /* rejected attempts (fixed: 0) */
+    int* status;           /* CHS_ST_* */
+    double* t_final;       /* time reached */
+} chs_report;
+
+/* phase-space dimension n of a problem, or -1 */
+int chaoticus_dim(const chs_problem* pb);
+/* rows of the sali / gali output of a FIXED-step run: 1 if sample_every <= 0, else
+ * ceil(n_steps / renorm_every) / sample_every + 1 (the last row is the final value) */
+long long chaoticus_n_samples(long long n_steps, int renorm_every, int sample_every);
+
+/* PAPER.md:47 (solver 1).  y DEVICE [n][n_ic] in/out. */
+int chaoticus_integrate_fixed(const chs_problem* pb, long long n_ic, double* y, double t0, double h,
+                              long long n_steps, const chs_report* rep, void* stream);
+
+/* PAPER.md:48, 53 (solver 2 + error computation).  st->adaptive must be 1. */
+int chaoticus_integrate_adaptive(const chs_problem* pb, long long n_ic, double* y, const chs_stepper* st,
+                                 const chs_report* rep, void* stream);
+
+/* PAPER.md:49-50 (solvers 3, 4) + PAPER.md:56: orbit + 2 deviation vectors, renormalised (not
+ * orthogonalised) after every renorm_every-th accepted step and at the end;
+ * SALI = min(|w1+w2|, |w1-w2|) of the unit vectors.
+ *  w        DEVICE [2][n][n_ic] in/out; normalised once on entry
+ *  sali     DEVICE [n_samples][n_ic]; row s < n_samples-1 = value after the
+ *           (s+1)*sample_every-th renormalisation, last row = value at the end.
+ *           sample_every must be 0 for adaptive runs (n_samples = 1).
+ *  lognorm  DEVICE [2][n_ic] or NULL; the run ADDS sum ln|w_v| of its renormalisations. */
+int chaoticus_sali(const chs_problem* pb, long long n_ic, double* y, double* w, const chs_stepper* st,
+                   int renorm_every, int sample_every, double* sali, double* lognorm,
+                   const chs_report* rep, void* stream);
+
+/* As chaoticus_sali with 2 <= k <= n vectors; GALI_k = product of the k singular values of the
+ * n x k matrix of unit deviation vectors. */
+int chaoticus_gali(const chs_problem* pb, long long n_ic, double* y, double* w, int k, const chs_stepper* st,
+                   int renorm_every, int sample_every, double* gali, double* lognorm,
+                   const chs_report* rep, void* stream);
+
+/* Arc-length Lagrangian descriptor (BASELINE.json configs[1]):
+ * M_+- = integral of |f(x(t))|_2 over [t0, t0 +- n_steps h], accumulated with the tableau's own
+ * quadrature, M += |h| sum_i b_i |k_i|.  y0 DEVICE [n][n_ic], NOT modified; h > 0;
+ * ld_fwd, ld_bwd DEVICE [n_ic], either may be NULL.  No variational equations. */
+int chaoticus_ld(const chs_problem* pb, long long n_ic, const double* y0, double t0, double h,
+                 long long n_steps, double* ld_fwd, double* ld_bwd, void* stream);
+
+/* PAPER.md:51-52 (solvers 5, 6): 1 <= k <= n vectors, modified Gram-Schmidt every
+ * renorm_every accepted steps and at the end (orthonormalised once on entry),
+ * S_v += ln r_vv.  lambda DEVICE [k][n_ic] = this run's sums / elapsed time (may be NULL);
+ * logsum DEVICE [k][n_ic] or NULL: the run ADDS its sums. */
+int chaoticus_lyap(const chs_problem* pb, long long n_ic, double* y, double* w, int k, const chs_stepper* st,
+                   int renorm_every, double* lambda, double* logsum, const chs_report* rep, void* stream);
+
+/* HOST-buffer forms (same meaning; all array arguments HOST, report members HOST or NULL).
+ * They allocate device scratch, copy in, run on an internal stream, copy out and synchronise. */
+int chaoticus_ld_host(const chs_problem* pb, long long n_ic, const double* y0, double t0, double h,
+                      long long n_steps, double* ld_fwd, double* ld_bwd);
+int chaoticus_sali_host(const chs_problem* pb, long long n_ic, double* y, double* w, const chs_stepper* st,
+                        int renorm_every, int sample_every, double* sali, double* lognorm,
+                        const chs_report* rep);
+int chaoticus_gali_host(const chs_problem* pb, long long n_ic, double* y, double* w, int k,
+                        const chs_stepper* st, int renorm_every, int sample_every, double* gali,
+                        double* lognorm, const chs_report* rep);
+int chaoticus_lyap_host(const chs_problem* pb, long long n_ic, double* y, double* w, int k,
+                        const chs_stepper* st, int renorm_every, double* lambda, double* logsum,
+                        const chs_report* rep);
+int chaoticus_integrate_host(const chs_problem* pb, long long n_ic, double* y, const chs_stepper* st,
+                             const chs_report* rep);
+
+/* Measurement aid: a register-only chain of dependent-free DFMAs,
+ * n_blocks x n_threads threads x iters x 16 DFMA each; out DEVICE [n_blocks*n_threads]
+ * (keeps the work alive).  Used by bench.py to measure the FP64 FMA peak of the device. */
+int chaoticus_dfma_probe(long long iters, int n_blocks, int n_threads, double* out, void* stream);
+
+/* Kernel launch shape the library would use for a call (for reporting): writes threads per
+ * block, blocks, lanes per trajectory, registers per thread, spill bytes.  what: 0 integrate,
+ * 1 sali, 2 gali, 3 ld, 4 lyap.  Returns CHS_EUNSUPPORTED if no kernel is compiled. */
+int chaoticus_kernel_info(const chs_problem* pb, int what, int k, int adaptive, long long n_ic, int* info5);
+
+const char* chaoticus_last_error(void); /* thread-local, static storage */
+int chaoticus_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CHAOTICUS_H */

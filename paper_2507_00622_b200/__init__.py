@@ -1,8 +1,20 @@
-"""chaoticus-b200: B200-native (sm_100a, FP64) hot path of arXiv 2507.00622 ("Chaoticus").
+"""paper_2507_00622_b200 -- B200-native (sm_100a, FP64) ensemble DOP8 integrator with chaos
+indicators (the hot path of arXiv 2507.00622).
 
-The product is the C-ABI library built from csrc/ (see include/chaoticus.h); `binding`
-is a thin ctypes layer with the same entry-point names.  Importing this package does not
-load the library; the first call does, and fails loudly if it is missing (there is no CPU
-fallback).
+    binding    ctypes binding of libchaoticus.so (C ABI: include/chaoticus.h); loaded lazily,
+               raises ImportError if the library has not been built (no CPU fallback)
+    workloads  seeded synthetic input generators (no arithmetic of the method)
+    build      in-tree nvcc build of the library
 """
-__all__ = ["binding", "workloads"]
+import importlib
+
+_API = ("integrate_fixed", "integrate_adaptive", "sali", "gali", "ld", "lyap", "ld_host", "sali_host", "gali_host",
+        "lyap_host", "integrate_host", "Report", "kernel_info", "dfma_probe", "dim", "n_samples", "version")
+
+
+def __getattr__(name):
+    if name in ("binding", "workloads", "build"):
+        return importlib.import_module(f"{__name__}.{name}")
+    if name in _API:
+        return getattr(importlib.import_module(f"{__name__}.binding"), name)
+    raise AttributeError(name)

@@ -1,0 +1,405 @@
+// chaoticus.cu -- C-ABI front end (include/chaoticus.h): argument checks, coefficient table,
+// dispatch to the compiled kernels.  No compute happens on the host; there is no CPU fallback.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+#include "../../include/chaoticus.h"
+#include "launch.h"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int rc, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return rc;
+}
+
+// coefficients premultiplied by powers of h (fixed step), or raw with h = 1 (adaptive)
+chs::Tab make_tab(double h) {
+    using namespace chs;
+    Tab t;
+    std::memset(&t, 0, sizeof t);
+    const double h2 = h * h;
+    for (int i = 0; i < 12; i++) {
+        for (int j = 0; j < 12; j++) {
+            t.a2[i][j] = coef::A2[i][j] * h2;
+            t.ap[i][j] = coef::A[i][j] * h;
+        }
+        t.cs[i] = coef::CS[i] * h;
+        t.bq[i] = coef::BQ[i] * h2;
+        t.bp[i] = coef::B[i] * h;
+        t.bl[i] = coef::B[i] * std::fabs(h);
+        t.e5q[i] = coef::E5Q[i];
+        t.e3q[i] = coef::E3Q[i];
+        t.e5p[i] = coef::E5[i];
+        t.e3p[i] = coef::E3[i];
+    }
+    t.h = h;
+    return t;
+}
+
+int dim_of(const chs_problem* pb, int* fput_n) {
+    if (fput_n) *fput_n = 0;
+    if (!pb) return -1;
+    switch (pb->system) {
+        case CHS_SYS_HENON_HEILES: return 4;
+        case CHS_SYS_COUPLED3: return (pb->params && pb->n_params >= 4) ? 6 : -1;
+        case CHS_SYS_FPUT: {
+            if (!pb->params || pb->n_params < 4) return -1;
+            const double Nd = pb->params[0];
+            if (!(Nd >= 1.0) || Nd > 4096.0 || Nd != std::floor(Nd)) return -1;
+            if (fput_n) *fput_n = (int)Nd;
+            return 2 * (int)Nd;
+        }
+    }
+    return -1;
+}
+
+int dispatch(const chs::LaunchReq& rq) {
+    int r;
+    if ((r = chs::try_launch_hh(rq)) != -1) return r;
+    if ((r = chs::try_launch_hh_ind(rq)) != -1) return r;
+    if ((r = chs::try_launch_hh_adapt(rq)) != -1) return r;
+    if ((r = chs::try_launch_c3(rq)) != -1) return r;
+    if ((r = chs::try_launch_c3_lyap(rq)) != -1) return r;
+    if ((r = chs::try_launch_fput(rq)) != -1) return r;
+    return -1;
+}
+
+int finish(int r, const chs::LaunchReq& rq) {
+    if (r == -1)
+        return fail(CHS_EUNSUPPORTED, "no compiled kernel for system=%d what=%d k=%d adaptive=%d", rq.system,
+                    rq.what, rq.k, rq.adaptive);
+    if (r != 0) return fail(CHS_ECUDA, "CUDA error %d: %s", r, cudaGetErrorString((cudaError_t)r));
+    return CHS_OK;
+}
+
+int check_stepper(const chs_stepper* st, int want_adaptive /* -1 any */) {
+    if (!st) return fail(CHS_EINVAL, "stepper is NULL");
+    if (want_adaptive >= 0 && (st->adaptive != 0) != (want_adaptive != 0))
+        return fail(CHS_EINVAL, "stepper.adaptive = %d not valid for this entry point", st->adaptive);
+    if (!st->adaptive) {
+        if (!(st->h != 0.0) || !std::isfinite(st->h)) return fail(CHS_EINVAL, "fixed step: h must be finite and != 0");
+        if (st->n_steps < 0) return fail(CHS_EINVAL, "fixed step: n_steps < 0");
+    } else {
+        if (!(st->rtol > 0.0) || !(st->atol > 0.0)) return fail(CHS_EINVAL, "adaptive: rtol and atol must be > 0");
+        if (!std::isfinite(st->t_end) || !std::isfinite(st->t0)) return fail(CHS_EINVAL, "adaptive: t0/t_end not finite");
+    }
+    return CHS_OK;
+}
+
+// common body of integrate / sali / gali / lyap
+int run_common(int what, const chs_problem* pb, long long n_ic, double* y, double* w, int k,
+               const chs_stepper* st, int renorm_every, int sample_every, double* series, double* logacc,
+               double* lambda, const chs_report* rep, void* stream, chs::KernelInfo* info) {
+    int fput_n = 0;
+    const int n = dim_of(pb, &fput_n);
+    if (n < 0) return fail(CHS_EINVAL, "unknown system or bad params");
+    if (n_ic < 0) return fail(CHS_EINVAL, "n_ic < 0");
+    int rc = check_stepper(st, -1);
+    if (rc) return rc;
+    if (!info) {
+        if (n_ic > 0 && !y) return fail(CHS_EINVAL, "y is NULL");
+        if (n_ic > 0 && k > 0 && !w) return fail(CHS_EINVAL, "w is NULL");
+    }
+    if (what == chs::WHAT_INTEGRATE && k != 0) return fail(CHS_EINVAL, "integrate: k must be 0");
+    if (what == chs::WHAT_SALI && k != 2) return fail(CHS_EINVAL, "sali: k must be 2");
+    if (what == chs::WHAT_GALI && (k < 2 || k > n)) return fail(CHS_EINVAL, "gali: need 2 <= k <= n");
+    if (what == chs::WHAT_LYAP && (k < 1 || k > n)) return fail(CHS_EINVAL, "lyap: need 1 <= k <= n");
+    if (what != chs::WHAT_INTEGRATE && renorm_every < 1) return fail(CHS_EINVAL, "renorm_every < 1");
+    if (sample_every < 0) return fail(CHS_EINVAL, "sample_every < 0");
+    if (st->adaptive && sample_every > 0) return fail(CHS_EINVAL, "adaptive runs: sample_every must be 0");
+    if ((what == chs::WHAT_SALI || what == chs::WHAT_GALI) && n_ic > 0 && !series && !info)
+        return fail(CHS_EINVAL, "indicator output is NULL");
+
+    chs::LaunchReq rq;
+    std::memset(&rq, 0, sizeof rq);
+    rq.system = pb->system;
+    rq.what = what;
+    rq.k = k;
+    rq.adaptive = st->adaptive ? 1 : 0;
+    rq.fput_n = fput_n;
+    rq.params = pb->params;
+    rq.n_params = pb->n_params;
+    rq.tab = make_tab(st->adaptive ? 1.0 : st->h);
+    rq.stream = (cudaStream_t)stream;
+    rq.info = info;
+    chs::RunArgs& a = rq.args;
+    a.n_ic = n_ic;
+    a.y = y;
+    a.w = w;
+    a.h = st->h;
+    a.n_steps = st->adaptive ? 0 : st->n_steps;
+    a.t0 = st->t0;
+    a.t_end = st->t_end;
+    a.rtol = st->rtol;
+    a.atol = st->atol;
+    a.h0 = st->h0;
+    a.max_steps = st->max_steps;
+    a.m = renorm_every < 1 ? 1 : renorm_every;
+    a.sample_every = sample_every;
+    a.n_samples = st->adaptive ? 1 : chaoticus_n_samples(st->n_steps, a.m, sample_every);
+    a.series = series;
+    a.logacc = logacc;
+    a.lambda = lambda;
+    if (rep) {
+        a.n_acc = rep->n_accepted;
+        a.n_rej = rep->n_rejected;
+        a.status = rep->status;
+        a.t_final = rep->t_final;
+    }
+    if (n_ic == 0 && !info) return CHS_OK;
+    return finish(dispatch(rq), rq);
+}
+
+}  // namespace
+
+extern "C" {
+
+int chaoticus_version(void) { return CHAOTICUS_VERSION; }
+const char* chaoticus_last_error(void) { return g_err; }
+
+int chaoticus_dim(const chs_problem* pb) { return dim_of(pb, nullptr); }
+
+long long chaoticus_n_samples(long long n_steps, int renorm_every, int sample_every) {
+    if (sample_every <= 0) return 1;
+    if (renorm_every < 1) renorm_every = 1;
+    const long long n_renorm = (n_steps + renorm_every - 1) / renorm_every;
+    return n_renorm / sample_every + 1;
+}
+
+int chaoticus_integrate_fixed(const chs_problem* pb, long long n_ic, double* y, double t0, double h,
+                              long long n_steps, const chs_report* rep, void* stream) {
+    chs_stepper st;
+    std::memset(&st, 0, sizeof st);
+    st.adaptive = 0;
+    st.t0 = t0;
+    st.h = h;
+    st.n_steps = n_steps;
+    return run_common(chs::WHAT_INTEGRATE, pb, n_ic, y, nullptr, 0, &st, 1, 0, nullptr, nullptr, nullptr, rep,
+                      stream, nullptr);
+}
+
+int chaoticus_integrate_adaptive(const chs_problem* pb, long long n_ic, double* y, const chs_stepper* st,
+                                 const chs_report* rep, void* stream) {
+    int rc = check_stepper(st, 1);
+    if (rc) return rc;
+    return run_common(chs::WHAT_INTEGRATE, pb, n_ic, y, nullptr, 0, st, 1, 0, nullptr, nullptr, nullptr, rep,
+                      stream, nullptr);
+}
+
+int chaoticus_sali(const chs_problem* pb, long long n_ic, double* y, double* w, const chs_stepper* st,
+                   int renorm_every, int sample_every, double* sali, double* lognorm, const chs_report* rep,
+                   void* stream) {
+    return run_common(chs::WHAT_SALI, pb, n_ic, y, w, 2, st, renorm_every, sample_every, sali, lognorm, nullptr,
+                      rep, stream, nullptr);
+}
+
+int chaoticus_gali(const chs_problem* pb, long long n_ic, double* y, double* w, int k, const chs_stepper* st,
+                   int renorm_every, int sample_every, double* gali, double* lognorm, const chs_report* rep,
+                   void* stream) {
+    return run_common(chs::WHAT_GALI, pb, n_ic, y, w, k, st, renorm_every, sample_every, gali, lognorm, nullptr,
+                      rep, stream, nullptr);
+}
+
+int chaoticus_lyap(const chs_problem* pb, long long n_ic, double* y, double* w, int k, const chs_stepper* st,
+                   int renorm_every, double* lambda, double* logsum, const chs_report* rep, void* stream) {
+    return run_common(chs::WHAT_LYAP, pb, n_ic, y, w, k, st, renorm_every, 0, nullptr, logsum, lambda, rep,
+                      stream, nullptr);
+}
+
+static int ld_common(const chs_problem* pb, long long n_ic, const double* y0, double t0, double h,
+                     long long n_steps, double* ld_fwd, double* ld_bwd, void* stream, chs::KernelInfo* info) {
+    (void)t0;  // autonomous systems: time is bookkeeping only
+    int fput_n = 0;
+    const int n = dim_of(pb, &fput_n);
+    if (n < 0) return fail(CHS_EINVAL, "unknown system or bad params");
+    if (n_ic < 0) return fail(CHS_EINVAL, "n_ic < 0");
+    if (!(h > 0.0) || !std::isfinite(h)) return fail(CHS_EINVAL, "ld: h must be > 0");
+    if (n_steps < 0) return fail(CHS_EINVAL, "ld: n_steps < 0");
+    if (!info && n_ic > 0 && !y0) return fail(CHS_EINVAL, "y0 is NULL");
+    if (!info && !ld_fwd && !ld_bwd) return CHS_OK;
+    chs::LaunchReq rq;
+    std::memset(&rq, 0, sizeof rq);
+    rq.system = pb->system;
+    rq.what = chs::WHAT_LD;
+    rq.k = 0;
+    rq.adaptive = 0;
+    rq.fput_n = fput_n;
+    rq.params = pb->params;
+    rq.n_params = pb->n_params;
+    rq.tab = make_tab(h);
+    rq.stream = (cudaStream_t)stream;
+    rq.info = info;
+    rq.args.n_ic = n_ic;
+    rq.args.y0 = y0;
+    rq.args.h = h;
+    rq.args.n_steps = n_steps;
+    rq.args.ld_fwd = ld_fwd;
+    rq.args.ld_bwd = ld_bwd;
+    rq.dir_first = ld_fwd ? 0 : 1;
+    rq.n_dirs = (info || (ld_fwd && ld_bwd)) ? 2 : 1;
+    if (info) rq.dir_first = 0;
+    if (n_ic == 0 && !info) return CHS_OK;
+    return finish(dispatch(rq), rq);
+}
+
+int chaoticus_ld(const chs_problem* pb, long long n_ic, const double* y0, double t0, double h, long long n_steps,
+                 double* ld_fwd, double* ld_bwd, void* stream) {
+    return ld_common(pb, n_ic, y0, t0, h, n_steps, ld_fwd, ld_bwd, stream, nullptr);
+}
+
+int chaoticus_kernel_info(const chs_problem* pb, int what, int k, int adaptive, long long n_ic, int* info5) {
+    if (!info5) return fail(CHS_EINVAL, "info5 is NULL");
+    chs::KernelInfo ki{0, 0, 0, 0, 0};
+    int rc;
+    if (what == chs::WHAT_LD) {
+        rc = ld_common(pb, n_ic, nullptr, 0.0, 1.0, 1, nullptr, nullptr, nullptr, &ki);
+    } else {
+        chs_stepper st;
+        std::memset(&st, 0, sizeof st);
+        st.adaptive = adaptive ? 1 : 0;
+        st.h = 1.0;
+        st.n_steps = 1;
+        st.t_end = 1.0;
+        st.rtol = st.atol = 1e-6;
+        rc = run_common(what, pb, n_ic, nullptr, nullptr, k, &st, 1, 0, nullptr, nullptr, nullptr, nullptr,
+                        nullptr, &ki);
+    }
+    if (rc) return rc;
+    info5[0] = ki.tpb;
+    info5[1] = ki.blocks;
+    info5[2] = ki.lanes;
+    info5[3] = ki.regs;
+    info5[4] = ki.spill_bytes;
+    return CHS_OK;
+}
+
+// ---- host-buffer forms ---------------------------------------------------------------------
+namespace {
+struct DevBuf {
+    void* p = nullptr;
+    size_t bytes = 0;
+    ~DevBuf() {
+        if (p) cudaFree(p);
+    }
+    cudaError_t alloc(size_t b) {
+        bytes = b;
+        return b ? cudaMalloc(&p, b) : cudaSuccess;
+    }
+};
+#define CK(x)                                                                                  \
+    do {                                                                                       \
+        cudaError_t e_ = (x);                                                                  \
+        if (e_ != cudaSuccess) {                                                               \
+            if (stream) cudaStreamDestroy(stream);                                             \
+            return fail(CHS_ECUDA, "CUDA error %d: %s", (int)e_, cudaGetErrorString(e_));      \
+        }                                                                                      \
+    } while (0)
+
+int run_host(int what, const chs_problem* pb, long long n_ic, double* y, double* w, int k, const chs_stepper* st,
+             int renorm_every, int sample_every, double* series, double* logacc, double* lambda,
+             const chs_report* rep) {
+    cudaStream_t stream = nullptr;
+    const int n = dim_of(pb, nullptr);
+    if (n < 0) return fail(CHS_EINVAL, "unknown system or bad params");
+    if (n_ic < 0) return fail(CHS_EINVAL, "n_ic < 0");
+    int rc = check_stepper(st, -1);
+    if (rc) return rc;
+    if (n_ic == 0) return CHS_OK;
+    if (!y || (k > 0 && !w)) return fail(CHS_EINVAL, "y or w is NULL");
+    const long long ns = st->adaptive ? 1 : chaoticus_n_samples(st->n_steps, renorm_every, sample_every);
+    const size_t by = sizeof(double) * (size_t)n * n_ic, bw = by * (size_t)k, bs = sizeof(double) * (size_t)ns * n_ic,
+                 bk = sizeof(double) * (size_t)k * n_ic;
+    DevBuf dy, dw, ds, dl, dlam, dacc, drej, dstat, dtf;
+    CK(cudaStreamCreate(&stream));
+    CK(dy.alloc(by));
+    CK(dw.alloc(bw));
+    if (series) CK(ds.alloc(bs));
+    if (logacc) CK(dl.alloc(bk));
+    if (lambda) CK(dlam.alloc(bk));
+    chs_report drep{nullptr, nullptr, nullptr, nullptr};
+    if (rep) {
+        if (rep->n_accepted) { CK(dacc.alloc(sizeof(long long) * n_ic)); drep.n_accepted = (long long*)dacc.p; }
+        if (rep->n_rejected) { CK(drej.alloc(sizeof(long long) * n_ic)); drep.n_rejected = (long long*)drej.p; }
+        if (rep->status) { CK(dstat.alloc(sizeof(int) * n_ic)); drep.status = (int*)dstat.p; }
+        if (rep->t_final) { CK(dtf.alloc(sizeof(double) * n_ic)); drep.t_final = (double*)dtf.p; }
+    }
+    CK(cudaMemcpyAsync(dy.p, y, by, cudaMemcpyHostToDevice, stream));
+    if (k > 0) CK(cudaMemcpyAsync(dw.p, w, bw, cudaMemcpyHostToDevice, stream));
+    if (logacc) CK(cudaMemcpyAsync(dl.p, logacc, bk, cudaMemcpyHostToDevice, stream));
+    rc = run_common(what, pb, n_ic, (double*)dy.p, (double*)dw.p, k, st, renorm_every, sample_every, (double*)ds.p,
+                    (double*)dl.p, (double*)dlam.p, &drep, stream, nullptr);
+    if (rc) {
+        cudaStreamDestroy(stream);
+        return rc;
+    }
+    CK(cudaMemcpyAsync(y, dy.p, by, cudaMemcpyDeviceToHost, stream));
+    if (k > 0) CK(cudaMemcpyAsync(w, dw.p, bw, cudaMemcpyDeviceToHost, stream));
+    if (series) CK(cudaMemcpyAsync(series, ds.p, bs, cudaMemcpyDeviceToHost, stream));
+    if (logacc) CK(cudaMemcpyAsync(logacc, dl.p, bk, cudaMemcpyDeviceToHost, stream));
+    if (lambda) CK(cudaMemcpyAsync(lambda, dlam.p, bk, cudaMemcpyDeviceToHost, stream));
+    if (rep) {
+        if (rep->n_accepted) CK(cudaMemcpyAsync(rep->n_accepted, dacc.p, sizeof(long long) * n_ic, cudaMemcpyDeviceToHost, stream));
+        if (rep->n_rejected) CK(cudaMemcpyAsync(rep->n_rejected, drej.p, sizeof(long long) * n_ic, cudaMemcpyDeviceToHost, stream));
+        if (rep->status) CK(cudaMemcpyAsync(rep->status, dstat.p, sizeof(int) * n_ic, cudaMemcpyDeviceToHost, stream));
+        if (rep->t_final) CK(cudaMemcpyAsync(rep->t_final, dtf.p, sizeof(double) * n_ic, cudaMemcpyDeviceToHost, stream));
+    }
+    CK(cudaStreamSynchronize(stream));
+    cudaStreamDestroy(stream);
+    return CHS_OK;
+}
+}  // namespace
+
+int chaoticus_ld_host(const chs_problem* pb, long long n_ic, const double* y0, double t0, double h,
+                      long long n_steps, double* ld_fwd, double* ld_bwd) {
+    cudaStream_t stream = nullptr;
+    const int n = dim_of(pb, nullptr);
+    if (n < 0) return fail(CHS_EINVAL, "unknown system or bad params");
+    if (n_ic < 0) return fail(CHS_EINVAL, "n_ic < 0");
+    if (n_ic == 0 || (!ld_fwd && !ld_bwd)) return CHS_OK;
+    if (!y0) return fail(CHS_EINVAL, "y0 is NULL");
+    DevBuf dy, df, db;
+    const size_t by = sizeof(double) * (size_t)n * n_ic, bo = sizeof(double) * (size_t)n_ic;
+    CK(cudaStreamCreate(&stream));
+    CK(dy.alloc(by));
+    if (ld_fwd) CK(df.alloc(bo));
+    if (ld_bwd) CK(db.alloc(bo));
+    CK(cudaMemcpyAsync(dy.p, y0, by, cudaMemcpyHostToDevice, stream));
+    int rc = chaoticus_ld(pb, n_ic, (const double*)dy.p, t0, h, n_steps, (double*)df.p, (double*)db.p, stream);
+    if (rc) {
+        cudaStreamDestroy(stream);
+        return rc;
+    }
+    if (ld_fwd) CK(cudaMemcpyAsync(ld_fwd, df.p, bo, cudaMemcpyDeviceToHost, stream));
+    if (ld_bwd) CK(cudaMemcpyAsync(ld_bwd, db.p, bo, cudaMemcpyDeviceToHost, stream));
+    CK(cudaStreamSynchronize(stream));
+    cudaStreamDestroy(stream);
+    return CHS_OK;
+}
+
+int chaoticus_sali_host(const chs_problem* pb, long long n_ic, double* y, double* w, const chs_stepper* st,
+                        int renorm_every, int sample_every, double* sali, double* lognorm, const chs_report* rep) {
+    return run_host(chs::WHAT_SALI, pb, n_ic, y, w, 2, st, renorm_every, sample_every, sali, lognorm, nullptr, rep);
+}
+int chaoticus_gali_host(const chs_problem* pb, long long n_ic, double* y, double* w, int k, const chs_stepper* st,
+                        int renorm_every, int sample_every, double* gali, double* lognorm, const chs_report* rep) {
+    return run_host(chs::WHAT_GALI, pb, n_ic, y, w, k, st, renorm_every, sample_every, gali, lognorm, nullptr, rep);
+}
+int chaoticus_lyap_host(const chs_problem* pb, long long n_ic, double* y, double* w, int k, const chs_stepper* st,
+                        int renorm_every, double* lambda, double* logsum, const chs_report* rep) {
+    return run_host(chs::WHAT_LYAP, pb, n_ic, y, w, k, st, renorm_every, 0, nullptr, logsum, lambda, rep);
+}
+int chaoticus_integrate_host(const chs_problem* pb, long long n_ic, double* y, const chs_stepper* st,
+                             const chs_report* rep) {
+    return run_host(chs::WHAT_INTEGRATE, pb, n_ic, y, nullptr, 0, st, 1, 0, nullptr, nullptr, nullptr, rep);
+}
+
+}  // extern "C"

@@ -1,0 +1,591 @@
+// col_kernels.cuh -- "column layout" step kernels (CUDA path, sm_100a).
+//
+// A trajectory's augmented state is 1 + K columns of n = 2 NDOF components: column 0 the orbit,
+// columns 1..K the deviation vectors.  The columns are dealt to a tile of L
+// consecutive lanes, CPL = ceil((1+K)/L) columns per lane:
+//   L = 1  : one trajectory per thread, everything in registers (Henon-Heiles, K <= 4);
+//   L > 1  : one column per lane (CPL = 1) for mid-size states (3-DoF Lyapunov spectrum:
+//            L = 8, lanes 0..6 busy); the orbit's stage coordinates are broadcast from lane 0
+//            by shuffle each stage, Gram-Schmidt broadcasts one column at a time.
+// HBM layout is structure-of-arrays (include/chaoticus.h); it is touched once at the start
+// and once at the end of a call, everything in between runs out of registers.
+#pragma once
+#include <cmath>
+#include "dop8_core.cuh"
+#include "systems.cuh"
+
+namespace chs {
+
+enum : int { MODE_NONE = 0, MODE_NORM = 1, MODE_MGS = 2 };
+enum : int { IND_NONE = 0, IND_SALI = 1, IND_GALI = 2 };
+
+struct RunArgs {
+    long long n_ic;
+    double* y;   // [n][n_ic]
+    double* w;   // [K][n][n_ic]
+    // fixed
+    double h;
+    long long n_steps;
+    // adaptive
+    double t0, t_end, rtol, atol, h0;
+    long long max_steps;
+    // renormalisation / sampling
+    int m;
+    int sample_every;
+    long long n_samples;
+    // outputs (may be null)
+    double* series;  // [n_samples][n_ic]
+    double* logacc;  // [K][n_ic]  +=
+    double* lambda;  // [K][n_ic]
+    long long* n_acc;
+    long long* n_rej;
+    int* status;
+    double* t_final;
+    // Lagrangian descriptor
+    const double* y0;
+    double* ld_fwd;
+    double* ld_bwd;
+};
+
+// one-sided (Hestenes) Jacobi on k columns of n components held by ONE thread; returns the
+// product of the singular values = GALI_k.  W is destroyed.
+template <int N, int KK>
+__device__ __forceinline__ double gali_thread(double (&W)[KK][N]) {
+    const double eps = 8.9e-16;  // 4 ulp: |a_p . a_q| <= eps |a_p| |a_q|  => orthogonal
+    for (int sweep = 0; sweep < 30; sweep++) {
+        bool rotated = false;
+#pragma unroll
+        for (int p = 0; p < KK - 1; p++)
+#pragma unroll
+            for (int q2 = p + 1; q2 < KK; q2++) {
+                double app = 0, aqq = 0, apq = 0;
+#pragma unroll
+                for (int c = 0; c < N; c++) {
+                    app = fma(W[p][c], W[p][c], app);
+                    aqq = fma(W[q2][c], W[q2][c], aqq);
+                    apq = fma(W[p][c], W[q2][c], apq);
+                }
+                if (fabs(apq) > eps * sqrt(app * aqq)) {
+                    rotated = true;
+                    double zeta = (aqq - app) / (2.0 * apq);
+                    double t = copysign(1.0, zeta) / (fabs(zeta) + sqrt(fma(zeta, zeta, 1.0)));
+                    double cs = rsqrt(fma(t, t, 1.0)), sn = cs * t;
+#pragma unroll
+                    for (int c = 0; c < N; c++) {
+                        double xp = W[p][c], xq = W[q2][c];
+                        W[p][c] = cs * xp - sn * xq;
+                        W[q2][c] = fma(sn, xp, cs * xq);
+                    }
+                }
+            }
+        if (!rotated) break;
+    }
+    double g = 1.0;
+#pragma unroll
+    for (int v = 0; v < KK; v++) {
+        double s = 0;
+#pragma unroll
+        for (int c = 0; c < N; c++) s = fma(W[v][c], W[v][c], s);
+        g *= sqrt(s);
+    }
+    return g;
+}
+
+// ---- per-lane view of one trajectory in the column layout -----------------------------------
+template <class Sys, int K, int L>
+struct Col {
+    static constexpr int ND = Sys::NDOF;
+    static constexpr int N = 2 * ND;
+    static constexpr int NCOL = 1 + K;
+    static constexpr int CPL = (NCOL + L - 1) / L;
+    static constexpr int NI = CPL * ND;
+    static constexpr int D = N * NCOL;
+
+    typename Sys::Params prm;
+    int lt;          // lane in tile
+    double s_lane;   // 1/2 on the orbit lane of a multi-lane tile, else 1
+    double q[NI], p[NI];
+    double lg[CPL];  // log accumulators of this lane's columns
+
+    __device__ __forceinline__ int col_of(int j) const { return lt * CPL + j; }
+    __device__ __forceinline__ bool is_dev(int j) const {
+        int c = col_of(j);
+        return c >= 1 && c < NCOL;
+    }
+
+    __device__ __forceinline__ void init(const typename Sys::Params& P) {
+        prm = P;
+        lt = (L == 1) ? 0 : (int)(threadIdx.x % L);
+        s_lane = (L > 1 && lt == 0) ? 0.5 : 1.0;
+#pragma unroll
+        for (int j = 0; j < CPL; j++) lg[j] = 0.0;
+    }
+
+    __device__ __forceinline__ void load(const double* y, const double* w, long long n_ic, long long ic,
+                                         double psign) {
+#pragma unroll
+        for (int j = 0; j < CPL; j++) {
+            const int c = col_of(j);
+#pragma unroll
+            for (int d = 0; d < ND; d++) {
+                double qq = 0.0, pp = 0.0;
+                if (c == 0) {
+                    qq = y[(long long)d * n_ic + ic];
+                    pp = psign * y[(long long)(ND + d) * n_ic + ic];
+                } else if (c < NCOL) {
+                    qq = w[((long long)(c - 1) * N + d) * n_ic + ic];
+                    pp = w[((long long)(c - 1) * N + ND + d) * n_ic + ic];
+                }
+                q[j * ND + d] = qq;
+                p[j * ND + d] = pp;
+            }
+        }
+    }
+    __device__ __forceinline__ void store(double* y, double* w, long long n_ic, long long ic, bool bad) const {
+#pragma unroll
+        for (int j = 0; j < CPL; j++) {
+            const int c = col_of(j);
+#pragma unroll
+            for (int d = 0; d < ND; d++) {
+                double qq = bad ? nan("") : q[j * ND + d], pp = bad ? nan("") : p[j * ND + d];
+                if (c == 0) {
+                    y[(long long)d * n_ic + ic] = qq;
+                    y[(long long)(ND + d) * n_ic + ic] = pp;
+                } else if (c < NCOL) {
+                    w[((long long)(c - 1) * N + d) * n_ic + ic] = qq;
+                    w[((long long)(c - 1) * N + ND + d) * n_ic + ic] = pp;
+                }
+            }
+        }
+    }
+
+    // force on all items at stage coordinates Q (Eq.(5) etc. + variational part)
+    __device__ __forceinline__ void force(const double (&Q)[NI], double (&F)[NI]) const {
+        double Qo[ND];
+#pragma unroll
+        for (int d = 0; d < ND; d++) Qo[d] = tile_bcast<L>(Q[d], 0);
+        if constexpr (L == 1) {
+            Sys::force(prm, Qo, &F[0]);
+            if constexpr (CPL > 1) {
+                const typename Sys::Hess H = Sys::hess(prm, Qo, 1.0);
+#pragma unroll
+                for (int j = 1; j < CPL; j++) Sys::apply(H, &Q[j * ND], &F[j * ND]);
+            }
+        } else {
+            const typename Sys::Hess H0 = Sys::hess(prm, Qo, s_lane);
+            Sys::apply(H0, &Q[0], &F[0]);
+            if constexpr (CPL > 1) {
+                const typename Sys::Hess H1 = Sys::hess(prm, Qo, 1.0);
+#pragma unroll
+                for (int j = 1; j < CPL; j++) Sys::apply(H1, &Q[j * ND], &F[j * ND]);
+            }
+        }
+    }
+
+    // value of component cc (0..N-1) of column `col` (compile-time), on every lane of the tile
+    template <int COL>
+    __device__ __forceinline__ double gather(int cc) const {
+        constexpr int owner = COL / CPL, j = COL % CPL;
+        const double v = (cc < ND) ? q[j * ND + cc] : p[j * ND + (cc - ND)];
+        return tile_bcast<L>(v, owner);
+    }
+
+    // Renormalisation: w_v <- w_v/|w_v|, lg += ln|w_v|.  Lane-local.
+    __device__ __forceinline__ void renorm(bool want_log, bool apply) {
+#pragma unroll
+        for (int j = 0; j < CPL; j++) {
+            if (L == 1 && j == 0) continue;  // the orbit
+            double s = 0.0;
+#pragma unroll
+            for (int d = 0; d < ND; d++) s = fma(q[j * ND + d], q[j * ND + d], fma(p[j * ND + d], p[j * ND + d], s));
+            const bool dev = is_dev(j) && apply;
+            const double a = sqrt(s);
+            const double inv = dev ? 1.0 / a : 1.0;
+#pragma unroll
+            for (int d = 0; d < ND; d++) {
+                q[j * ND + d] *= inv;
+                p[j * ND + d] *= inv;
+            }
+            if (want_log && dev) lg[j] += log(a);
+        }
+    }
+
+    // Modified Gram-Schmidt ("QR factorization"; BASELINE configs[3]):
+    // for v = 1..K: r_vv = |w_v|, q_v = w_v/r_vv, lg_v += ln r_vv, then every later column
+    // w_u -= (q_v . w_u) q_v  (right-looking order: the same operations on each column, in the
+    // same order, as the textbook left-looking loop).  Warp-convergent; `apply` predicates.
+    __device__ __forceinline__ void mgs(bool want_log, bool apply) {
+        static_for<1, NCOL>([&](auto vc) {
+            constexpr int v = decltype(vc)::value;
+            constexpr int owner = v / CPL, jv = v % CPL;
+            double wq[ND], wp[ND];
+            double s = 0.0;
+#pragma unroll
+            for (int d = 0; d < ND; d++) {
+                wq[d] = tile_bcast<L>(q[jv * ND + d], owner);
+                wp[d] = tile_bcast<L>(p[jv * ND + d], owner);
+            }
+#pragma unroll
+            for (int d = 0; d < ND; d++) s = fma(wq[d], wq[d], s);
+#pragma unroll
+            for (int d = 0; d < ND; d++) s = fma(wp[d], wp[d], s);
+            const double r = sqrt(s), inv = 1.0 / r;
+#pragma unroll
+            for (int d = 0; d < ND; d++) {
+                wq[d] *= inv;
+                wp[d] *= inv;
+            }
+            const bool mine = apply && (lt == owner);
+            if (mine) {
+#pragma unroll
+                for (int d = 0; d < ND; d++) {
+                    q[jv * ND + d] = wq[d];
+                    p[jv * ND + d] = wp[d];
+                }
+                if (want_log) lg[jv] += log(r);
+            }
+#pragma unroll
+            for (int j = 0; j < CPL; j++) {
+                const int c = col_of(j);
+                if ((L == 1) ? (j > v) : (c > v && c < NCOL && apply)) {
+                    double dot = 0.0;
+#pragma unroll
+                    for (int d = 0; d < ND; d++) dot = fma(wq[d], q[j * ND + d], dot);
+#pragma unroll
+                    for (int d = 0; d < ND; d++) dot = fma(wp[d], p[j * ND + d], dot);
+#pragma unroll
+                    for (int d = 0; d < ND; d++) {
+                        q[j * ND + d] = fma(-dot, wq[d], q[j * ND + d]);
+                        p[j * ND + d] = fma(-dot, wp[d], p[j * ND + d]);
+                    }
+                }
+            }
+        });
+    }
+
+    template <int MODE>
+    __device__ __forceinline__ void do_renorm(bool want_log, bool apply) {
+        if constexpr (MODE == MODE_NORM) renorm(want_log, apply);
+        if constexpr (MODE == MODE_MGS) mgs(want_log, apply);
+    }
+
+    // SALI / GALI_k of the current unit vectors; same on all lanes
+    template <int IND>
+    __device__ __forceinline__ double indicator() const {
+        if constexpr (IND == IND_SALI) {
+            double sp = 0.0, sm = 0.0;
+#pragma unroll
+            for (int cc = 0; cc < N; cc++) {
+                const double a = gather<1>(cc), b = gather<(K >= 2 ? 2 : 1)>(cc);
+                const double u = a + b, d = a - b;
+                sp = fma(u, u, sp);
+                sm = fma(d, d, sm);
+            }
+            sp = sqrt(sp);
+            sm = sqrt(sm);
+            return sp < sm ? sp : sm;
+        } else if constexpr (IND == IND_GALI) {
+            double W[K][N];
+            static_for<0, K>([&](auto vc) {
+                constexpr int v = decltype(vc)::value;
+#pragma unroll
+                for (int cc = 0; cc < N; cc++) W[v][cc] = gather<v + 1>(cc);
+            });
+            return gali_thread<N, K>(W);
+        } else {
+            return 0.0;
+        }
+    }
+
+    __device__ __forceinline__ bool finite_all() const {
+        bool ok = true;
+#pragma unroll
+        for (int c = 0; c < NI; c++) ok = ok && isfinite(q[c]) && isfinite(p[c]);
+        return !tile_any<L>(!ok);
+    }
+
+    __device__ __forceinline__ void on_mask(bool (&on)[NI]) const {
+#pragma unroll
+        for (int j = 0; j < CPL; j++)
+#pragma unroll
+            for (int d = 0; d < ND; d++) on[j * ND + d] = col_of(j) < NCOL;
+    }
+
+    // Starting step of the adaptive solver (item 6)
+    __device__ __forceinline__ double initial_step(double interval, double dir, double rtol, double atol) const {
+        if (interval == 0.0) return 0.0;
+        bool on[NI];
+        on_mask(on);
+        double F0[NI], F1[NI], q1[NI], p1[NI];
+        force(q, F0);
+        double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+        for (int c = 0; c < NI; c++) {
+            const double iq = 1.0 / fma(fabs(q[c]), rtol, atol), ip = 1.0 / fma(fabs(p[c]), rtol, atol);
+            if (on[c]) {
+                s0 += (q[c] * iq) * (q[c] * iq) + (p[c] * ip) * (p[c] * ip);
+                s1 += (p[c] * iq) * (p[c] * iq) + (F0[c] * ip) * (F0[c] * ip);
+            }
+        }
+        const double d0 = sqrt(tile_sum<L>(s0) / D), d1 = sqrt(tile_sum<L>(s1) / D);
+        double ha = (d0 < 1e-5 || d1 < 1e-5) ? 1e-6 : 0.01 * d0 / d1;
+        ha = fmin(ha, interval);
+#pragma unroll
+        for (int c = 0; c < NI; c++) {
+            q1[c] = fma(ha * dir, p[c], q[c]);
+            p1[c] = fma(ha * dir, F0[c], p[c]);
+        }
+        force(q1, F1);
+        double s2 = 0.0;
+#pragma unroll
+        for (int c = 0; c < NI; c++) {
+            const double iq = 1.0 / fma(fabs(q[c]), rtol, atol), ip = 1.0 / fma(fabs(p[c]), rtol, atol);
+            const double dq = (p1[c] - p[c]) * iq, dp = (F1[c] - F0[c]) * ip;
+            if (on[c]) s2 += dq * dq + dp * dp;
+        }
+        const double d2 = sqrt(tile_sum<L>(s2) / D) / ha;
+        double hb;
+        if (d1 <= 1e-15 && d2 <= 1e-15) hb = fmax(1e-6, 1e-3 * ha);
+        else hb = root8(0.01 / fmax(d1, d2));
+        return fmin(fmin(100.0 * ha, hb), interval);
+    }
+};
+
+// functors handed to dop8_stages (plain structs: generic lambdas with array-reference
+// parameters of dependent extent crash cudafe++ 12.9)
+template <class C>
+struct ForceFn {
+    const C& s;
+    __device__ __forceinline__ void operator()(const double (&Q)[C::NI], double (&F)[C::NI]) const { s.force(Q, F); }
+};
+struct NoHook {
+    template <class I, class FF>
+    __device__ __forceinline__ void operator()(I, const FF&) const {}
+};
+// LD quadrature: after stage i, M += |h| b_i |(P_i, F_i)|_2
+template <class C>
+struct LdHook {
+    const Tab& tab;
+    const C& s;
+    double& M;
+    template <int i>
+    __device__ __forceinline__ void operator()(Int<i>, const double (&F)[12][C::NI]) const {
+        if constexpr (coef::B[i] != 0.0) {
+            double n2 = 0.0;
+#pragma unroll
+            for (int c = 0; c < C::NI; c++) {
+                double P = s.p[c];
+                static_for<0, i>([&](auto jc) {
+                    constexpr int j = decltype(jc)::value;
+                    if constexpr (coef::A[i][j] != 0.0) P = fma(tab.ap[i][j], F[j][c], P);
+                });
+                n2 = fma(P, P, fma(F[i][c], F[i][c], n2));
+            }
+            M = fma(tab.bl[i], sqrt(n2), M);
+        }
+    }
+};
+
+// ---- the run kernel: fixed or adaptive, with renormalisation / indicator ----------------------
+template <class Sys, int K, int L, int MODE, int IND, bool ADAPT, int TPB, int MINB>
+__global__ void __launch_bounds__(TPB, MINB)
+col_run_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, const RunArgs a) {
+    using C = Col<Sys, K, L>;
+    constexpr int NI = C::NI;
+    const long long gt = (long long)blockIdx.x * TPB + threadIdx.x;
+    const long long traj = gt / L;
+    const bool valid = traj < a.n_ic;
+    const long long ic = valid ? traj : a.n_ic - 1;  // padding lanes shadow the last trajectory
+
+    C s;
+    s.init(prm);
+    s.load(a.y, a.w, a.n_ic, ic, 1.0);
+    const bool want_log = (a.logacc != nullptr) || (a.lambda != nullptr);
+    s.template do_renorm<MODE>(false, true);  // on entry: no log accumulated
+
+    const ForceFn<C> force{s};
+    const NoHook nohook{};
+
+    long long n_acc = 0, n_rej = 0;
+    int status = ST_OK;
+    double t = a.t0;
+    long long slot = 0;
+
+    if constexpr (!ADAPT) {
+        int cd = a.m, sd = a.sample_every;
+        for (long long st = 1; st <= a.n_steps; ++st) {
+            double F[12][NI];
+            dop8_stages<NI, true>(tab, 0.0, 0.0, s.q, s.p, F, force, nohook);
+            double qn[NI], pn[NI];
+            dop8_solution<NI, true>(tab, 0.0, 0.0, s.q, s.p, F, qn, pn);
+#pragma unroll
+            for (int c = 0; c < NI; c++) {
+                s.q[c] = qn[c];
+                s.p[c] = pn[c];
+            }
+            if constexpr (MODE != MODE_NONE) {
+                if (--cd == 0 || st == a.n_steps) {
+                    cd = a.m;
+                    s.template do_renorm<MODE>(want_log, true);
+                    if constexpr (IND != IND_NONE) {
+                        if (a.sample_every > 0 && --sd == 0) {
+                            sd = a.sample_every;
+                            if (slot < a.n_samples - 1) {
+                                const double v = s.template indicator<IND>();
+                                if (valid && s.lt == 0) a.series[slot * a.n_ic + ic] = v;
+                                slot++;
+                            }
+                        }
+                    }
+                }
+            }
+        }
+        n_acc = a.n_steps;
+        t = a.t0 + (double)a.n_steps * a.h;
+    } else {
+        const double dir = (a.t_end >= a.t0) ? 1.0 : -1.0;
+        double h_abs = a.h0 > 0.0 ? a.h0 : s.initial_step(fabs(a.t_end - a.t0), dir, a.rtol, a.atol);
+        long long attempts = 0;
+        bool rejected = false;
+        double min_step = 0.0;
+        int cd = a.m;
+        bool on[NI];
+        s.on_mask(on);
+        while (true) {
+            bool active = valid && status == ST_OK && dir * (a.t_end - t) > 0.0;
+            if (!__any_sync(0xffffffffu, active)) break;
+            if (!rejected) {
+                min_step = 10.0 * fabs(nextafter(t, dir * INFINITY) - t);
+                h_abs = fmax(h_abs, min_step);
+            }
+            if (active && h_abs < min_step) {
+                status = ST_UNDERFLOW;
+                active = false;
+            }
+            if (active && a.max_steps > 0 && attempts >= a.max_steps) {
+                status = ST_MAXSTEPS;
+                active = false;
+            }
+            attempts += active ? 1 : 0;
+            double t_new = t + h_abs * dir;
+            if (dir * (t_new - a.t_end) > 0.0) t_new = a.t_end;  // land exactly on t_end
+            const double h = t_new - t;
+            const double h_try = fabs(h);
+
+            double F[12][NI];
+            dop8_stages<NI, false>(tab, h, h * h, s.q, s.p, F, force, nohook);
+            double qn[NI], pn[NI];
+            dop8_solution<NI, false>(tab, h, h * h, s.q, s.p, F, qn, pn);
+            double S5, S3;
+            dop8_error_sums<NI>(tab, h, s.q, s.p, qn, pn, F, a.rtol, a.atol, on, S5, S3);
+            S5 = tile_sum<L>(S5);
+            S3 = tile_sum<L>(S3);
+            const double err = (S5 == 0.0 && S3 == 0.0) ? 0.0 : h_try * S5 / sqrt((S5 + 0.01 * S3) * (double)C::D);
+
+            bool ren = false;
+            if (active) {
+                if (err < 1.0) {
+                    double factor = (err == 0.0) ? 10.0 : fmin(10.0, 0.9 / root8(err));
+                    if (rejected) factor = fmin(factor, 1.0);
+                    h_abs = h_try * factor;
+                    t = t_new;
+#pragma unroll
+                    for (int c = 0; c < NI; c++) {
+                        s.q[c] = qn[c];
+                        s.p[c] = pn[c];
+                    }
+                    n_acc++;
+                    rejected = false;
+                    const bool at_end = !(dir * (a.t_end - t) > 0.0);
+                    if (MODE != MODE_NONE && (--cd == 0 || at_end)) {
+                        cd = a.m;
+                        ren = true;
+                    }
+                } else if (err >= 1.0) {
+                    h_abs = h_try * fmax(0.2, 0.9 / root8(err));
+                    rejected = true;
+                    n_rej++;
+                } else {
+                    status = ST_NONFINITE;
+                }
+            }
+            if constexpr (MODE != MODE_NONE) {
+                if (__any_sync(0xffffffffu, ren)) s.template do_renorm<MODE>(want_log, ren);
+            }
+            const bool fin = s.finite_all();  // tile-wide, warp-convergent
+            if (active && !fin) status = ST_NONFINITE;
+        }
+    }
+    // ---- outputs ------------------------------------------------------------------------------
+    bool bad = !s.finite_all();
+    if (ADAPT) bad = tile_any<L>(status != ST_OK) || bad;
+    if (bad && status == ST_OK) status = ST_NONFINITE;
+    double ind = 0.0;
+    if constexpr (IND != IND_NONE) ind = s.template indicator<IND>();
+    if (!valid) return;
+    s.store(a.y, a.w, a.n_ic, ic, bad);
+    if constexpr (K > 0) {
+        const double elapsed = t - a.t0;
+#pragma unroll
+        for (int j = 0; j < C::CPL; j++) {
+            if (s.is_dev(j)) {
+                const long long o = (long long)(s.col_of(j) - 1) * a.n_ic + ic;
+                if (a.logacc) a.logacc[o] = bad ? nan("") : a.logacc[o] + s.lg[j];
+                if (a.lambda) a.lambda[o] = (bad || elapsed == 0.0) ? nan("") : s.lg[j] / elapsed;
+            }
+        }
+    }
+    if (s.lt == 0) {
+        if constexpr (IND != IND_NONE) {
+            if (a.series) {
+                a.series[(a.n_samples - 1) * a.n_ic + ic] = bad ? nan("") : ind;
+                if (bad)
+                    for (long long r = slot; r < a.n_samples - 1; r++) a.series[r * a.n_ic + ic] = nan("");
+            }
+        }
+        if (a.n_acc) a.n_acc[ic] = n_acc;
+        if (a.n_rej) a.n_rej[ic] = n_rej;
+        if (a.status) a.status[ic] = status;
+        if (a.t_final) a.t_final[ic] = t;
+    }
+}
+
+// ---- Lagrangian descriptor kernel (BASELINE configs[1]) ------------
+// One thread per (direction, IC).  The backward pass is the forward pass of the momentum-
+// reversed initial condition: H is even in p, so stepping (q, p) with -h and stepping (q, -p)
+// with +h give mirror-image states bit for bit and the same |f|.
+// M += |h| sum_i b_i |k_i|_2 with k_i = (P_i, F_i) the stage derivative; P_i is formed only at
+// the 8 stages with b_i != 0.
+template <class Sys, int TPB, int MINB>
+__global__ void __launch_bounds__(TPB, MINB)
+col_ld_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, const RunArgs a, int dir_first,
+              int n_dirs) {
+    using C = Col<Sys, 0, 1>;
+    constexpr int NI = C::NI;
+    const long long gt = (long long)blockIdx.x * TPB + threadIdx.x;
+    if (gt >= a.n_ic * n_dirs) return;
+    const int dsel = dir_first + (int)(gt / a.n_ic);  // 0 forward, 1 backward
+    const long long ic = gt % a.n_ic;
+    C s;
+    s.init(prm);
+    s.load(a.y0, nullptr, a.n_ic, ic, dsel == 0 ? 1.0 : -1.0);
+    double M = 0.0;
+    const ForceFn<C> force{s};
+    LdHook<C> hook{tab, s, M};
+    for (long long st = 0; st < a.n_steps; ++st) {
+        double F[12][NI];
+        dop8_stages<NI, true>(tab, 0.0, 0.0, s.q, s.p, F, force, hook);
+        double qn[NI], pn[NI];
+        dop8_solution<NI, true>(tab, 0.0, 0.0, s.q, s.p, F, qn, pn);
+#pragma unroll
+        for (int c = 0; c < NI; c++) {
+            s.q[c] = qn[c];
+            s.p[c] = pn[c];
+        }
+    }
+    const bool ok = s.finite_all();
+    double* out = dsel == 0 ? a.ld_fwd : a.ld_bwd;
+    out[ic] = ok ? M : nan("");
+}
+
+}  // namespace chs

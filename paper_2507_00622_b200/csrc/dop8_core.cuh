@@ -1,0 +1,180 @@
+// dop8_core.cuh -- the DOP8 step in separable form, layout-agnostic (CUDA path, sm_100a).
+//
+// PAPER.md:43 ("the 8th order ODE solver given in [51]"), PAPER.md:47-53 (fixed "DOP 8",
+// adaptive "DOP 8(5)", per-step error).  DESIGN.md "Separable form":
+// every system on the path has H = |p|^2/2 + V(q), so the q-half of every stage derivative is
+// the p-stage value and is never stored.  A lane holds NI independent (q, p) component pairs
+// ("items": orbit coordinates and/or deviation-vector coordinates); the only coupling between
+// items is inside the force functor.  With F_l = force(Q_l):
+//     Q_i = q + cs_i h p + h^2 sum_l A2_il F_l,   q+ = q + h p + h^2 sum_l BQ_l F_l,
+//     p+ = p + h sum_l B_l F_l.
+// All stage loops are compile-time (static_for over integral constants) so that state and
+// stage forces live in registers and structural zeros of the tableau cost nothing.
+#pragma once
+#include <cuda_runtime.h>
+#include <type_traits>
+#include "dop8_coeffs.h"
+
+namespace chs {
+
+template <int I> using Int = std::integral_constant<int, I>;
+
+template <int B, int E, class F>
+__device__ __forceinline__ void static_for(F&& f) {
+    if constexpr (B < E) {
+        f(Int<B>{});
+        static_for<B + 1, E>(f);
+    }
+}
+
+// Coefficients as the kernels read them (a __grid_constant__ kernel parameter, i.e. constant
+// bank operands of the DFMAs).  Fixed step: premultiplied by powers of h on the host.
+// Adaptive: raw (h = 1) and the per-trajectory h is applied in registers.
+struct Tab {
+    double a2[12][12];  // h^2 A2
+    double ap[12][12];  // h A           (P stages; Lagrangian descriptor only)
+    double cs[12];      // h rowsum(A)
+    double bq[12];      // h^2 b^T A
+    double bp[12];      // h b
+    double bl[12];      // |h| b         (LD quadrature weights)
+    double e5q[12], e3q[12];  // (adaptive, raw) E5^T A, E3^T A
+    double e5p[12], e3p[12];  // (adaptive, raw) E5, E3
+    double h;                 // signed step (fixed) or 1
+};
+
+// ---- tile helpers: a trajectory is owned by L consecutive lanes (L = 1, 2, 4, 8, 16, 32) ----
+template <int L>
+__device__ __forceinline__ double tile_bcast(double x, int src_lane_in_tile) {
+    if constexpr (L == 1) return x;
+    else return __shfl_sync(0xffffffffu, x, src_lane_in_tile, L);
+}
+template <int L>
+__device__ __forceinline__ double tile_sum(double x) {  // butterfly: identical on all lanes
+    if constexpr (L > 1) {
+#pragma unroll
+        for (int d = L / 2; d >= 1; d >>= 1) x += __shfl_xor_sync(0xffffffffu, x, d, L);
+    }
+    return x;
+}
+template <int L>
+__device__ __forceinline__ bool tile_any(bool b) {
+    if constexpr (L == 1) return b;
+    else {
+        unsigned m = __ballot_sync(0xffffffffu, b);
+        unsigned lane = threadIdx.x & 31u;
+        unsigned tmask = (L == 32) ? 0xffffffffu : (((1u << L) - 1u) << (lane & ~(unsigned)(L - 1)));
+        return (m & tmask) != 0u;
+    }
+}
+
+// ---- stages -------------------------------------------------------------------------------
+// force(Q, Fout): evaluates the NI force components at the stage coordinates Q.
+// hook(Int<i>, F): called after stage i's force is available (used by the LD quadrature).
+template <int NI, bool PREMUL, class Force, class Hook>
+__device__ __forceinline__ void dop8_stages(const Tab& tab, double h, double h2, const double (&q)[NI],
+                                            const double (&p)[NI], double (&F)[12][NI], Force&& force,
+                                            Hook&& hook) {
+    force(q, F[0]);
+    hook(Int<0>{}, F);
+    static_for<1, 12>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        double Q[NI];
+#pragma unroll
+        for (int c = 0; c < NI; c++) {
+            if constexpr (PREMUL) {
+                double acc = fma(tab.cs[i], p[c], q[c]);
+                static_for<0, i>([&](auto lc) {
+                    constexpr int l = decltype(lc)::value;
+                    if constexpr (coef::A2[i][l] != 0.0) acc = fma(tab.a2[i][l], F[l][c], acc);
+                });
+                Q[c] = acc;
+            } else {
+                double base = fma(h * tab.cs[i], p[c], q[c]);
+                if constexpr (i == 1) {
+                    Q[c] = base;  // row 2 of A.A is empty
+                } else {
+                    double s = tab.a2[i][0] * F[0][c];
+                    static_for<1, i>([&](auto lc) {
+                        constexpr int l = decltype(lc)::value;
+                        if constexpr (coef::A2[i][l] != 0.0) s = fma(tab.a2[i][l], F[l][c], s);
+                    });
+                    Q[c] = fma(h2, s, base);
+                }
+            }
+        }
+        force(Q, F[i]);
+        hook(ic, F);
+    });
+}
+
+// 8th-order solution from the stage forces
+template <int NI, bool PREMUL>
+__device__ __forceinline__ void dop8_solution(const Tab& tab, double h, double h2, const double (&q)[NI],
+                                              const double (&p)[NI], const double (&F)[12][NI],
+                                              double (&qn)[NI], double (&pn)[NI]) {
+#pragma unroll
+    for (int c = 0; c < NI; c++) {
+        if constexpr (PREMUL) {
+            double aq = fma(tab.h, p[c], q[c]);
+            double ap = p[c];
+            static_for<0, 12>([&](auto lc) {
+                constexpr int l = decltype(lc)::value;
+                if constexpr (coef::BQ[l] != 0.0) aq = fma(tab.bq[l], F[l][c], aq);
+                if constexpr (coef::B[l] != 0.0) ap = fma(tab.bp[l], F[l][c], ap);
+            });
+            qn[c] = aq;
+            pn[c] = ap;
+        } else {
+            double sq = tab.bq[0] * F[0][c];
+            double sp = tab.bp[0] * F[0][c];
+            static_for<1, 12>([&](auto lc) {
+                constexpr int l = decltype(lc)::value;
+                if constexpr (coef::BQ[l] != 0.0) sq = fma(tab.bq[l], F[l][c], sq);
+                if constexpr (coef::B[l] != 0.0) sp = fma(tab.bp[l], F[l][c], sp);
+            });
+            qn[c] = fma(h2, sq, fma(h, p[c], q[c]));
+            pn[c] = fma(h, sp, p[c]);
+        }
+    }
+}
+
+// Embedded error sums of one attempted step:
+// this lane's contribution to S5 = sum_c (e5_c/scale_c)^2 and S3 likewise, over its 2 NI
+// components, scale_c = atol + rtol max(|y_c|, |y+_c|).  Raw tableau (h applied here).
+// `on[c]` masks padding items.
+template <int NI>
+__device__ __forceinline__ void dop8_error_sums(const Tab& tab, double h, const double (&q)[NI],
+                                                const double (&p)[NI], const double (&qn)[NI],
+                                                const double (&pn)[NI], const double (&F)[12][NI],
+                                                double rtol, double atol, const bool (&on)[NI], double& S5,
+                                                double& S3) {
+    S5 = 0.0;
+    S3 = 0.0;
+#pragma unroll
+    for (int c = 0; c < NI; c++) {
+        double s5q = tab.e5q[0] * F[0][c], s3q = tab.e3q[0] * F[0][c];
+        double s5p = tab.e5p[0] * F[0][c], s3p = tab.e3p[0] * F[0][c];
+        static_for<1, 12>([&](auto lc) {
+            constexpr int l = decltype(lc)::value;
+            if constexpr (coef::E5Q[l] != 0.0) s5q = fma(tab.e5q[l], F[l][c], s5q);
+            if constexpr (coef::E3Q[l] != 0.0) s3q = fma(tab.e3q[l], F[l][c], s3q);
+            if constexpr (coef::E5[l] != 0.0) s5p = fma(tab.e5p[l], F[l][c], s5p);
+            if constexpr (coef::E3[l] != 0.0) s3p = fma(tab.e3p[l], F[l][c], s3p);
+        });
+        double iq = 1.0 / fma(rtol, fmax(fabs(q[c]), fabs(qn[c])), atol);
+        double ip = 1.0 / fma(rtol, fmax(fabs(p[c]), fabs(pn[c])), atol);
+        double a = h * s5q * iq, b = s5p * ip, c3 = h * s3q * iq, d3 = s3p * ip;
+        if (on[c]) {
+            S5 = fma(a, a, fma(b, b, S5));
+            S3 = fma(c3, c3, fma(d3, d3, S3));
+        }
+    }
+}
+
+// per-trajectory status words (include/chaoticus.h CHS_ST_*)
+enum : int { ST_OK = 0, ST_NONFINITE = 1, ST_UNDERFLOW = 2, ST_MAXSTEPS = 3 };
+
+// x^(1/8) by three square roots (the controller's exponent)
+__device__ __forceinline__ double root8(double x) { return sqrt(sqrt(sqrt(x))); }
+
+}  // namespace chs

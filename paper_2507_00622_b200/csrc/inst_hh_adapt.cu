@@ -1,0 +1,12 @@
+// inst_hh_adapt.cu -- Henon-Heiles, adaptive DOP8(5): plain integration, SALI, GALI_k, Lyapunov.
+#include "launch.h"
+namespace chs {
+int try_launch_hh_adapt(const LaunchReq& rq) {
+    if (CHS_MATCH(0, WHAT_INTEGRATE, 0, 1)) return run_col<HenonHeiles, 0, 1, MODE_NONE, IND_NONE, true, 128, 4>(rq);
+    if (CHS_MATCH(0, WHAT_SALI, 2, 1)) return run_col<HenonHeiles, 2, 1, MODE_NORM, IND_SALI, true, 128, 1>(rq);
+    if (CHS_MATCH(0, WHAT_GALI, 2, 1)) return run_col<HenonHeiles, 2, 1, MODE_NORM, IND_GALI, true, 128, 1>(rq);
+    if (CHS_MATCH(0, WHAT_LYAP, 1, 1)) return run_col<HenonHeiles, 1, 1, MODE_MGS, IND_NONE, true, 128, 2>(rq);
+    if (CHS_MATCH(0, WHAT_LYAP, 2, 1)) return run_col<HenonHeiles, 2, 1, MODE_MGS, IND_NONE, true, 128, 1>(rq);
+    return -1;
+}
+}  // namespace chs

@@ -1,0 +1,79 @@
+// launch.h -- host-side launch request shared by the C-ABI front end (chaoticus.cu) and the
+// translation units that instantiate the kernels (inst_*.cu).  CUDA path only.
+#pragma once
+#include <cuda_runtime.h>
+#include "col_kernels.cuh"
+
+namespace chs {
+
+enum : int { WHAT_INTEGRATE = 0, WHAT_SALI = 1, WHAT_GALI = 2, WHAT_LD = 3, WHAT_LYAP = 4 };
+
+struct KernelInfo {
+    int tpb, blocks, lanes, regs, spill_bytes;
+};
+
+struct LaunchReq {
+    int system, what, k, adaptive;
+    int fput_n;            // FPUT only: particles
+    const double* params;  // host
+    int n_params;
+    Tab tab;
+    RunArgs args;
+    cudaStream_t stream;
+    KernelInfo* info;  // non-null: report the launch shape, launch nothing
+    // LD: which directions
+    int dir_first, n_dirs;
+};
+
+// each returns -1 if it has no kernel for the request, else a cudaError_t (0 = success)
+int try_launch_hh(const LaunchReq& rq);
+int try_launch_hh_ind(const LaunchReq& rq);
+int try_launch_hh_adapt(const LaunchReq& rq);
+int try_launch_c3(const LaunchReq& rq);
+int try_launch_c3_lyap(const LaunchReq& rq);
+int try_launch_fput(const LaunchReq& rq);
+
+template <class Kern>
+inline int finish_launch(const LaunchReq& rq, Kern kern, int tpb, int lanes, long long n_threads) {
+    long long blocks = (n_threads + tpb - 1) / tpb;
+    if (rq.info) {
+        cudaFuncAttributes at;
+        cudaError_t e = cudaFuncGetAttributes(&at, kern);
+        if (e != cudaSuccess) return (int)e;
+        *rq.info = KernelInfo{tpb, (int)blocks, lanes, at.numRegs, (int)at.localSizeBytes};
+        return 0;
+    }
+    return -2;  // caller launches
+}
+
+template <class Sys, int K, int L, int MODE, int IND, bool ADAPT, int TPB, int MINB>
+inline int run_col(const LaunchReq& rq) {
+    typename Sys::Params prm;
+    if (!Sys::make_params(rq.params, rq.n_params, prm)) return (int)cudaErrorInvalidValue;
+    auto kern = col_run_kernel<Sys, K, L, MODE, IND, ADAPT, TPB, MINB>;
+    const long long n_threads = rq.args.n_ic * L;
+    int r = finish_launch(rq, kern, TPB, L, n_threads);
+    if (r != -2) return r;
+    const long long blocks = (n_threads + TPB - 1) / TPB;
+    if (blocks == 0) return 0;
+    kern<<<(unsigned)blocks, TPB, 0, rq.stream>>>(rq.tab, prm, rq.args);
+    return (int)cudaGetLastError();
+}
+
+template <class Sys, int TPB, int MINB>
+inline int run_ld(const LaunchReq& rq) {
+    typename Sys::Params prm;
+    if (!Sys::make_params(rq.params, rq.n_params, prm)) return (int)cudaErrorInvalidValue;
+    auto kern = col_ld_kernel<Sys, TPB, MINB>;
+    const long long n_threads = rq.args.n_ic * rq.n_dirs;
+    int r = finish_launch(rq, kern, TPB, 1, n_threads);
+    if (r != -2) return r;
+    const long long blocks = (n_threads + TPB - 1) / TPB;
+    if (blocks == 0) return 0;
+    kern<<<(unsigned)blocks, TPB, 0, rq.stream>>>(rq.tab, prm, rq.args, rq.dir_first, rq.n_dirs);
+    return (int)cudaGetLastError();
+}
+
+#define CHS_MATCH(SYSID, WHAT, KK, AD) (rq.system == (SYSID) && rq.what == (WHAT) && rq.k == (KK) && rq.adaptive == (AD))
+
+}  // namespace chs

@@ -1,0 +1,366 @@
+"""GPU parity tests: the CUDA path (through the C ABI, via the ctypes binding) against the CPU
+oracle on the same seeded inputs, element by element.  Sizes: the oracle finishes each in
+seconds, ensembles span several thread blocks and end in a ragged tail.
+
+Tolerances (BASELINE.json north_star):
+  states, fixed step, t <= 10 Lyapunov times : |dy|_2 / |y|_2 <= 1e-10 per trajectory
+  indicators on regular orbits               : relative 1e-8
+The truth is the oracle in x86 80-bit long double ("f80"); the double oracle is reported too.
+"""
+import numpy as np
+import pytest
+
+from paper_2507_00622_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+HH, C3, FPUT = W.SYS_HENON_HEILES, W.SYS_COUPLED3, W.SYS_FPUT
+TOL_STATE = 1e-10
+TOL_IND = 1e-8
+
+
+@pytest.fixture(scope="module")
+def chs():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2507_00622_b200 import binding
+    return binding
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def rel_state(y_gpu, y_ref):
+    """per-trajectory |dy|_2/|y|_2 over the leading axis (components)."""
+    y_gpu = y_gpu.reshape(-1, y_gpu.shape[-1])
+    y_ref = y_ref.reshape(-1, y_ref.shape[-1])
+    return np.linalg.norm(y_gpu - y_ref, axis=0) / np.linalg.norm(y_ref, axis=0)
+
+
+# ---------------------------------------------------------------------------- plain integration
+@pytest.mark.parametrize("h", [0.01, -0.01])
+def test_integrate_fixed_hh(chs, orc, h):
+    y0 = W.hh_grid(0.125, 19, 17)  # 323 ICs: 2 full blocks + ragged tail
+    yo = y0.copy()
+    orc.integrate_fixed(HH, None, yo, 0.0, h, 3000, precision="f80")
+    yg = dev(y0)
+    rep = chs.Report(y0.shape[1], "cuda")
+    chs.integrate_fixed(HH, None, yg, 0.0, h, 3000, report=rep)
+    r = rel_state(yg.cpu().numpy(), yo)
+    assert r.max() <= TOL_STATE, r.max()
+    assert (rep.status.cpu().numpy() == 0).all()
+    assert (rep.n_accepted.cpu().numpy() == 3000).all()
+    np.testing.assert_allclose(rep.t_final.cpu().numpy(), 3000 * h, rtol=1e-15)
+
+
+def test_integrate_fixed_coupled3_exact(chs, orc):
+    """eps = 0: uncoupled oscillators, closed form q cos(wt) + p/w sin(wt)."""
+    prm = W.coupled3_params(0.0)
+    y0 = W.coupled3_ics(200, seed=5, E=0.1, eps=0.0)
+    yg = dev(y0)
+    chs.integrate_fixed(C3, prm, yg, 0.0, 0.01, 5000)
+    t = 50.0
+    w = prm[:3][:, None]
+    q = y0[:3] * np.cos(w * t) + y0[3:] / w * np.sin(w * t)
+    p = -y0[:3] * w * np.sin(w * t) + y0[3:] * np.cos(w * t)
+    r = rel_state(yg.cpu().numpy(), np.concatenate([q, p]))
+    assert r.max() <= 1e-11, r.max()
+
+
+def test_integrate_fixed_coupled3(chs, orc):
+    prm = W.coupled3_params(0.1)
+    y0 = W.coupled3_ics(300, seed=1)
+    yo = y0.copy()
+    orc.integrate_fixed(C3, prm, yo, 0.0, 0.01, 2000, precision="f80")
+    yg = dev(y0)
+    chs.integrate_fixed(C3, prm, yg, 0.0, 0.01, 2000)
+    assert rel_state(yg.cpu().numpy(), yo).max() <= TOL_STATE
+
+
+def test_resume_bit_identical(chs):
+    y0 = W.hh_grid(0.125, 16, 16)
+    a = dev(y0)
+    b = dev(y0)
+    chs.integrate_fixed(HH, None, a, 0.0, 0.01, 1000)
+    chs.integrate_fixed(HH, None, b, 0.0, 0.01, 400)
+    chs.integrate_fixed(HH, None, b, 4.0, 0.01, 600)
+    assert (a == b).all().item()
+
+
+def test_empty_and_single(chs, orc):
+    import torch
+    y = torch.empty((4, 0), dtype=torch.float64, device="cuda")
+    chs.integrate_fixed(HH, None, y, 0.0, 0.01, 10)
+    f, b = chs.ld(HH, None, y, 0.0, 0.01, 10)
+    assert f.numel() == 0 and b.numel() == 0
+    y1 = W.hh_grid(0.125, 1, 1)
+    yo = y1.copy()
+    orc.integrate_fixed(HH, None, yo, 0.0, 0.01, 100, precision="f80")
+    yg = dev(y1)
+    chs.integrate_fixed(HH, None, yg, 0.0, 0.01, 100)
+    assert rel_state(yg.cpu().numpy(), yo).max() <= TOL_STATE
+
+
+def test_argument_errors(chs):
+    import torch
+    y = torch.zeros((4, 8), dtype=torch.float64, device="cuda")
+    with pytest.raises(chs.ChaoticusError):
+        chs.integrate_fixed(HH, None, y, 0.0, 0.0, 10)            # h = 0
+    with pytest.raises(chs.ChaoticusError):
+        chs.integrate_adaptive(HH, None, y, 0.0, 1.0, 0.0, 1e-9)  # rtol = 0
+    with pytest.raises(chs.ChaoticusError):
+        chs.integrate_fixed(7, None, y, 0.0, 0.01, 10)            # unknown system
+    w = torch.zeros((2, 4, 8), dtype=torch.float64, device="cuda")
+    with pytest.raises(chs.ChaoticusError):
+        chs.sali(HH, None, y, w, renorm_every=0, h=0.01, n_steps=10)
+    with pytest.raises(ValueError):
+        chs.integrate_fixed(HH, None, y[:, ::2], 0.0, 0.01, 10)    # non-contiguous
+
+
+def test_nonfinite_status(chs):
+    """An escaping Henon-Heiles orbit (E far above 1/6) overflows: status 1, outputs NaN."""
+    y0 = W.hh_grid(0.125, 4, 4)
+    y0[:, 3] = [0.0, 3.0, 0.0, 5.0]   # far outside the bounded region
+    yg = dev(y0)
+    rep = chs.Report(16, "cuda")
+    chs.integrate_fixed(HH, None, yg, 0.0, 0.05, 4000, report=rep)
+    st = rep.status.cpu().numpy()
+    out = yg.cpu().numpy()
+    assert st[3] == chs.ST_NONFINITE and np.isnan(out[:, 3]).all()
+    ok = np.delete(np.arange(16), 3)
+    assert (st[ok] == 0).all() and np.isfinite(out[:, ok]).all()
+
+
+# ---------------------------------------------------------------------------- Lagrangian descriptor
+def test_ld_hh(chs, orc):
+    y0 = W.hh_grid(0.125, 37, 37)  # 1369 ICs
+    fo, bo = orc.ld(HH, None, y0, 0.0, 0.01, 1500, precision="f80")
+    f, b = chs.ld(HH, None, dev(y0), 0.0, 0.01, 1500)
+    f, b = f.cpu().numpy(), b.cpu().numpy()
+    assert np.abs(f / fo - 1).max() <= TOL_IND and np.abs(b / bo - 1).max() <= TOL_IND
+    # time-reversal + reflection symmetry on the py-symmetric grid: M-(y,py) = M+(y,-py)
+    F = f.reshape(37, 37)
+    B = b.reshape(37, 37)
+    assert np.abs(B - F[:, ::-1]).max() <= 1e-12
+    # one direction only
+    f2, none = chs.ld(HH, None, dev(y0), 0.0, 0.01, 1500, backward=False)
+    assert none is None and (f2.cpu().numpy() == f).all()
+    none, b2 = chs.ld(HH, None, dev(y0), 0.0, 0.01, 1500, forward=False)
+    assert (b2.cpu().numpy() == b).all()
+
+
+def test_ld_harmonic_closed_form(chs):
+    """All omega = 1, eps = 0: |f| = sqrt(2E) is constant, M+ = M- = tau sqrt(2E)."""
+    prm = np.array([1.0, 1.0, 1.0, 0.0])
+    rng = np.random.default_rng(3)
+    y0 = np.ascontiguousarray(rng.uniform(-1, 1, size=(6, 257)))
+    E = 0.5 * (y0 ** 2).sum(0)
+    f, b = chs.ld(C3, prm, dev(y0), 0.0, 0.01, 2000)
+    exact = 20.0 * np.sqrt(2 * E)
+    assert np.abs(f.cpu().numpy() / exact - 1).max() <= 1e-12
+    assert np.abs(b.cpu().numpy() / exact - 1).max() <= 1e-12
+
+
+def test_ld_host_entry(chs, orc):
+    y0 = W.hh_grid(0.125, 12, 12)
+    f = np.empty(144)
+    b = np.empty(144)
+    chs.ld_host(HH, None, y0, 0.0, 0.01, 500, f, b)
+    fd, bd = chs.ld(HH, None, dev(y0), 0.0, 0.01, 500)
+    assert (fd.cpu().numpy() == f).all() and (bd.cpu().numpy() == b).all()
+
+
+# ---------------------------------------------------------------------------- SALI, fixed step
+def _sali_case(n_side=24, n_steps=2000):
+    cfg = W.config("C1", n_ic=n_side * n_side)
+    return cfg["y"], cfg["w"]
+
+
+def test_sali_fixed_hh(chs, orc):
+    y0, w0 = _sali_case()
+    n_ic = y0.shape[1]
+    yo, wo, lo = y0.copy(), w0.copy(), np.zeros((2, n_ic))
+    ro = orc.sali(HH, None, yo, wo, renorm_every=1, sample_every=500, lognorm=lo, h=0.01, n_steps=2000,
+                  precision="f80")
+    yg, wg, lg = dev(y0), dev(w0), dev(np.zeros((2, n_ic)))
+    sg = chs.sali(HH, None, yg, wg, renorm_every=1, sample_every=500, lognorm=lg, h=0.01, n_steps=2000)
+    sg = sg.cpu().numpy()
+    so = ro["series"]
+    assert sg.shape == so.shape == (5, n_ic)
+    assert rel_state(yg.cpu().numpy(), yo).max() <= TOL_STATE
+    # t = 20 is far below 10 Lyapunov times for every orbit: all SALI values are O(1e-3..1)
+    assert so.min() > 1e-6
+    assert np.abs(sg / so - 1).max() <= TOL_IND
+    assert np.abs(wg.cpu().numpy() - wo).max() <= 1e-9
+    assert np.abs(lg.cpu().numpy() - lo).max() <= 1e-9
+    # unit vectors on return
+    nrm = np.linalg.norm(wg.cpu().numpy(), axis=1)
+    assert np.abs(nrm - 1).max() <= 1e-14
+
+
+def test_sali_renorm_interval_and_tail(chs, orc):
+    """m = 7 does not divide n_steps = 1000: a final renormalisation happens at the end."""
+    y0, w0 = _sali_case(10)
+    n_ic = y0.shape[1]
+    yo, wo = y0.copy(), w0.copy()
+    ro = orc.sali(HH, None, yo, wo, renorm_every=7, sample_every=10, h=0.01, n_steps=1000, precision="f80")
+    yg, wg = dev(y0), dev(w0)
+    sg = chs.sali(HH, None, yg, wg, renorm_every=7, sample_every=10, h=0.01, n_steps=1000).cpu().numpy()
+    assert sg.shape == ro["series"].shape
+    assert np.abs(sg / ro["series"] - 1).max() <= TOL_IND
+    assert np.abs(wg.cpu().numpy() - wo).max() <= 1e-10
+
+
+def test_sali_resume(chs):
+    y0, w0 = _sali_case(12)
+    a_y, a_w = dev(y0), dev(w0)
+    b_y, b_w = dev(y0), dev(w0)
+    sa = chs.sali(HH, None, a_y, a_w, renorm_every=5, h=0.01, n_steps=1000)
+    chs.sali(HH, None, b_y, b_w, renorm_every=5, h=0.01, n_steps=500)
+    sb = chs.sali(HH, None, b_y, b_w, renorm_every=5, t0=5.0, h=0.01, n_steps=500)
+    assert (a_y == b_y).all().item() and (a_w == b_w).all().item() and (sa == sb).all().item()
+
+
+def test_sali_host_entry(chs):
+    y0, w0 = _sali_case(9)
+    yh, wh, sh = y0.copy(), w0.copy(), np.empty((1, 81))
+    chs.sali_host(HH, None, yh, wh, sh, renorm_every=1, h=0.01, n_steps=300)
+    yg, wg = dev(y0), dev(w0)
+    sg = chs.sali(HH, None, yg, wg, renorm_every=1, h=0.01, n_steps=300)
+    assert (sg.cpu().numpy() == sh).all() and (yg.cpu().numpy() == yh).all() and (wg.cpu().numpy() == wh).all()
+
+
+def test_sali_coupled3_tile(chs, orc):
+    """Same entry point on the 3-DoF system: 4-lane tile per trajectory (orbit, w1, w2, idle)."""
+    prm = W.coupled3_params(0.1)
+    y0 = W.coupled3_ics(150, seed=1)
+    w0 = W.deviation_vectors(150, 2, 6, 7, "unit")
+    yo, wo = y0.copy(), w0.copy()
+    ro = orc.sali(C3, prm, yo, wo, renorm_every=3, sample_every=100, h=0.01, n_steps=1500, precision="f80")
+    yg, wg = dev(y0), dev(w0)
+    sg = chs.sali(C3, prm, yg, wg, renorm_every=3, sample_every=100, h=0.01, n_steps=1500).cpu().numpy()
+    assert rel_state(yg.cpu().numpy(), yo).max() <= TOL_STATE
+    assert np.abs(sg / ro["series"] - 1).max() <= TOL_IND
+    assert np.abs(wg.cpu().numpy() - wo).max() <= 1e-9
+
+
+# ---------------------------------------------------------------------------- GALI / Lyapunov, Henon-Heiles
+@pytest.mark.parametrize("k", [2, 3, 4])
+def test_gali_fixed_hh(chs, orc, k):
+    y0 = W.hh_grid(0.125, 13, 11)
+    n_ic = y0.shape[1]
+    w0 = W.deviation_vectors(n_ic, k, 4, 11, "orthonormal")
+    yo, wo = y0.copy(), w0.copy()
+    ro = orc.gali(HH, None, yo, wo, renorm_every=5, sample_every=40, h=0.01, n_steps=1000, precision="f80")
+    yg, wg = dev(y0), dev(w0)
+    gg = chs.gali(HH, None, yg, wg, renorm_every=5, sample_every=40, h=0.01, n_steps=1000).cpu().numpy()
+    go = ro["series"]
+    assert gg.shape == go.shape
+    assert rel_state(yg.cpu().numpy(), yo).max() <= TOL_STATE
+    big = go > 1e-12
+    assert np.abs(gg[big] / go[big] - 1).max() <= TOL_IND
+    assert np.abs(gg[~big] - go[~big]).max(initial=0.0) <= 1e-14
+
+
+@pytest.mark.parametrize("k", [1, 2, 3, 4])
+def test_lyap_fixed_hh(chs, orc, k):
+    y0 = W.hh_grid(0.125, 11, 13)
+    n_ic = y0.shape[1]
+    w0 = W.deviation_vectors(n_ic, k, 4, 12, "raw")   # not orthonormal: entry MGS is exercised
+    yo, wo, so = y0.copy(), w0.copy(), np.zeros((k, n_ic))
+    ro = orc.lyap(HH, None, yo, wo, renorm_every=10, logsum=so, h=0.01, n_steps=2005, precision="f80")
+    yg, wg, sg = dev(y0), dev(w0), dev(np.zeros((k, n_ic)))
+    lam = chs.lyap(HH, None, yg, wg, renorm_every=10, logsum=sg, h=0.01, n_steps=2005).cpu().numpy()
+    T = 20.05
+    den = np.maximum(np.abs(ro["lam"]).max(0), 1.0 / T)
+    assert (np.abs(lam - ro["lam"]) / den).max() <= TOL_IND
+    assert np.abs(sg.cpu().numpy() - so).max() <= 1e-9
+    assert rel_state(yg.cpu().numpy(), yo).max() <= TOL_STATE
+    assert np.abs(wg.cpu().numpy() - wo).max() <= 1e-9
+    # orthonormal on return
+    Wm = np.transpose(wg.cpu().numpy(), (2, 0, 1))       # [ic, k, n]
+    G = Wm @ np.transpose(Wm, (0, 2, 1))
+    assert np.abs(G - np.eye(k)).max() <= 1e-13
+
+
+# ---------------------------------------------------------------------------- 3-DoF Lyapunov spectrum (C4 shape)
+def test_lyap_coupled3_full_spectrum(chs, orc):
+    cfg = W.config("C4", n_ic=203)
+    y0, w0, prm = cfg["y"], cfg["w"], cfg["params"]
+    n_ic = y0.shape[1]
+    yo, wo = y0.copy(), w0.copy()
+    ro = orc.lyap(C3, prm, yo, wo, renorm_every=10, h=0.01, n_steps=3000, precision="f80")
+    yg, wg = dev(y0), dev(w0)
+    lam = chs.lyap(C3, prm, yg, wg, renorm_every=10, h=0.01, n_steps=3000).cpu().numpy()
+    T = 30.0
+    den = np.maximum(np.abs(ro["lam"]).max(0), 1.0 / T)
+    assert (np.abs(lam - ro["lam"]) / den).max() <= TOL_IND
+    assert rel_state(yg.cpu().numpy(), yo).max() <= TOL_STATE
+    assert np.abs(wg.cpu().numpy() - wo).max() <= 1e-9
+    assert np.abs(lam.sum(0)).max() <= 1e-12            # Liouville: sum of exponents = 0
+
+
+def test_lyap_coupled3_mle_matches_first_exponent(chs):
+    cfg = W.config("C4", n_ic=64)
+    y0, w0, prm = cfg["y"], cfg["w"], cfg["params"]
+    lam6 = chs.lyap(C3, prm, dev(y0), dev(w0), renorm_every=10, h=0.01, n_steps=2000).cpu().numpy()
+    lam1 = chs.lyap(C3, prm, dev(y0), dev(w0[:1].copy()), renorm_every=10, h=0.01, n_steps=2000).cpu().numpy()
+    assert np.abs(lam1[0] - lam6[0]).max() <= 1e-12
+
+
+# ---------------------------------------------------------------------------- adaptive DOP8(5)
+def test_integrate_adaptive_hh(chs, orc):
+    y0 = W.hh_grid(1.0 / 6.0, 15, 14)
+    n_ic = y0.shape[1]
+    yo = y0.copy()
+    ro = orc.integrate_adaptive(HH, None, yo, 0.0, 50.0, 1e-12, 1e-12, precision="f80")
+    yg = dev(y0)
+    rep = chs.Report(n_ic, "cuda")
+    chs.integrate_adaptive(HH, None, yg, 0.0, 50.0, 1e-12, 1e-12, report=rep)
+    assert (rep.status.cpu().numpy() == 0).all()
+    assert (rep.t_final.cpu().numpy() == 50.0).all()
+    # both are solutions to tolerance 1e-12 of the same ODE; step sequences may differ by
+    # isolated accept/reject flips (R16), so the state tolerance is the solver's own
+    # global error level, not round-off
+    assert rel_state(yg.cpu().numpy(), yo).max() <= 2e-9
+    na, nr = rep.n_accepted.cpu().numpy(), rep.n_rejected.cpu().numpy()
+    assert abs(na.sum() / ro["n_accepted"].sum() - 1) <= 5e-3
+    assert (np.abs(na - ro["n_accepted"]) <= 2).mean() >= 0.9
+    assert abs(int(nr.sum()) - int(ro["n_rejected"].sum())) <= 0.1 * ro["n_rejected"].sum() + 5
+
+
+def test_sali_adaptive_hh(chs, orc):
+    cfg = W.config("C3", n_ic=14 * 14)
+    y0, w0 = cfg["y"], cfg["w"]
+    n_ic = y0.shape[1]
+    yo, wo = y0.copy(), w0.copy()
+    ro = orc.sali(HH, None, yo, wo, renorm_every=1, adaptive=True, t_end=60.0, rtol=1e-12, atol=1e-12,
+                  precision="f80")
+    yg, wg = dev(y0), dev(w0)
+    rep = chs.Report(n_ic, "cuda")
+    sg = chs.sali(HH, None, yg, wg, renorm_every=1, adaptive=True, t_end=60.0, rtol=1e-12, atol=1e-12,
+                  report=rep).cpu().numpy()
+    so = ro["series"]
+    assert (rep.status.cpu().numpy() == 0).all()
+    assert rel_state(yg.cpu().numpy(), yo).max() <= 1e-8
+    reg = so[0] > 1e-4
+    assert reg.sum() > 0.5 * n_ic
+    assert np.abs(sg[0][reg] / so[0][reg] - 1).max() <= 1e-6
+    assert abs(rep.n_accepted.cpu().numpy().sum() / ro["n_accepted"].sum() - 1) <= 5e-3
+
+
+def test_adaptive_max_steps_and_backward(chs, orc):
+    y0 = W.hh_grid(0.125, 6, 6)
+    yg = dev(y0)
+    rep = chs.Report(36, "cuda")
+    chs.integrate_adaptive(HH, None, yg, 0.0, 100.0, 1e-10, 1e-10, max_steps=20, report=rep)
+    assert (rep.status.cpu().numpy() == chs.ST_MAXSTEPS).all() and np.isnan(yg.cpu().numpy()).all()
+    # backward in time (t_end < t0) against the oracle
+    yo = y0.copy()
+    orc.integrate_adaptive(HH, None, yo, 0.0, -20.0, 1e-11, 1e-11, precision="f80")
+    yg = dev(y0)
+    chs.integrate_adaptive(HH, None, yg, 0.0, -20.0, 1e-11, 1e-11)
+    assert rel_state(yg.cpu().numpy(), yo).max() <= 1e-8
