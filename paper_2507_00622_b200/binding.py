@@ -99,7 +99,7 @@ def dim(system, params=None):
 
 
 def _dim(pb):
-    n = _dim(pb)
+    n = _lib.chaoticus_dim(C.byref(pb))
     if n < 0:
         raise ChaoticusError(f"unknown system id {pb.system} or bad parameter list")
     return n

@@ -221,7 +221,10 @@ def test_sali_resume(chs):
     sa = chs.sali(HH, None, a_y, a_w, renorm_every=5, h=0.01, n_steps=1000)
     chs.sali(HH, None, b_y, b_w, renorm_every=5, h=0.01, n_steps=500)
     sb = chs.sali(HH, None, b_y, b_w, renorm_every=5, t0=5.0, h=0.01, n_steps=500)
-    assert (a_y == b_y).all().item() and (a_w == b_w).all().item() and (sa == sb).all().item()
+    # the orbit does not depend on the deviation vectors: bit-identical.  The second call's entry
+    # normalisation divides the already-unit vectors by |w| = 1 +- ulp: last-digit differences.
+    assert (a_y == b_y).all().item()
+    assert (a_w - b_w).abs().max().item() <= 1e-14 and ((sa - sb).abs() / sa).max().item() <= 1e-13
 
 
 def test_sali_host_entry(chs):
