@@ -92,16 +92,18 @@ __device__ __forceinline__ double gali_thread(double (&W)[KK][N]) {
 }
 
 // ---- per-lane view of one trajectory in the column layout -----------------------------------
-template <class Sys, int K, int L>
+template <class Sys, int K_, int L_>
 struct Col {
+    static constexpr int K = K_, L = L_;
     static constexpr int ND = Sys::NDOF;
     static constexpr int N = 2 * ND;
     static constexpr int NCOL = 1 + K;
     static constexpr int CPL = (NCOL + L - 1) / L;
     static constexpr int NI = CPL * ND;
     static constexpr int D = N * NCOL;
+    using Params = typename Sys::Params;
 
-    typename Sys::Params prm;
+    Params prm;
     int lt;          // lane in tile
     double s_lane;   // 1/2 on the orbit lane of a multi-lane tile, else 1
     double q[NI], p[NI];
@@ -311,45 +313,61 @@ struct Col {
             for (int d = 0; d < ND; d++) on[j * ND + d] = col_of(j) < NCOL;
     }
 
-    // Starting step of the adaptive solver (item 6)
-    __device__ __forceinline__ double initial_step(double interval, double dir, double rtol, double atol) const {
-        if (interval == 0.0) return 0.0;
-        bool on[NI];
-        on_mask(on);
-        double F0[NI], F1[NI], q1[NI], p1[NI];
-        force(q, F0);
-        double s0 = 0.0, s1 = 0.0;
+    // accumulated logs -> logacc (+=) and lambda (= sum / elapsed); each lane writes its own columns
+    __device__ __forceinline__ void store_logs(const RunArgs& a, long long ic, bool bad, double elapsed) const {
+        if constexpr (K > 0) {
 #pragma unroll
-        for (int c = 0; c < NI; c++) {
-            const double iq = 1.0 / fma(fabs(q[c]), rtol, atol), ip = 1.0 / fma(fabs(p[c]), rtol, atol);
-            if (on[c]) {
-                s0 += (q[c] * iq) * (q[c] * iq) + (p[c] * ip) * (p[c] * ip);
-                s1 += (p[c] * iq) * (p[c] * iq) + (F0[c] * ip) * (F0[c] * ip);
+            for (int j = 0; j < CPL; j++) {
+                if (is_dev(j)) {
+                    const long long o = (long long)(col_of(j) - 1) * a.n_ic + ic;
+                    if (a.logacc) a.logacc[o] = bad ? nan("") : a.logacc[o] + lg[j];
+                    if (a.lambda) a.lambda[o] = (bad || elapsed == 0.0) ? nan("") : lg[j] / elapsed;
+                }
             }
         }
-        const double d0 = sqrt(tile_sum<L>(s0) / D), d1 = sqrt(tile_sum<L>(s1) / D);
-        double ha = (d0 < 1e-5 || d1 < 1e-5) ? 1e-6 : 0.01 * d0 / d1;
-        ha = fmin(ha, interval);
-#pragma unroll
-        for (int c = 0; c < NI; c++) {
-            q1[c] = fma(ha * dir, p[c], q[c]);
-            p1[c] = fma(ha * dir, F0[c], p[c]);
-        }
-        force(q1, F1);
-        double s2 = 0.0;
-#pragma unroll
-        for (int c = 0; c < NI; c++) {
-            const double iq = 1.0 / fma(fabs(q[c]), rtol, atol), ip = 1.0 / fma(fabs(p[c]), rtol, atol);
-            const double dq = (p1[c] - p[c]) * iq, dp = (F1[c] - F0[c]) * ip;
-            if (on[c]) s2 += dq * dq + dp * dp;
-        }
-        const double d2 = sqrt(tile_sum<L>(s2) / D) / ha;
-        double hb;
-        if (d1 <= 1e-15 && d2 <= 1e-15) hb = fmax(1e-6, 1e-3 * ha);
-        else hb = root8(0.01 / fmax(d1, d2));
-        return fmin(fmin(100.0 * ha, hb), interval);
     }
 };
+
+// Starting step of the adaptive solver (item 6), any layout S
+template <class S>
+__device__ __forceinline__ double initial_step(const S& s, double interval, double dir, double rtol, double atol) {
+    constexpr int NI = S::NI, L = S::L, D = S::D;
+    if (interval == 0.0) return 0.0;
+    bool on[NI];
+    s.on_mask(on);
+    double F0[NI], F1[NI], q1[NI], p1[NI];
+    s.force(s.q, F0);
+    double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+    for (int c = 0; c < NI; c++) {
+        const double iq = 1.0 / fma(fabs(s.q[c]), rtol, atol), ip = 1.0 / fma(fabs(s.p[c]), rtol, atol);
+        if (on[c]) {
+            s0 += (s.q[c] * iq) * (s.q[c] * iq) + (s.p[c] * ip) * (s.p[c] * ip);
+            s1 += (s.p[c] * iq) * (s.p[c] * iq) + (F0[c] * ip) * (F0[c] * ip);
+        }
+    }
+    const double d0 = sqrt(tile_sum<L>(s0) / D), d1 = sqrt(tile_sum<L>(s1) / D);
+    double ha = (d0 < 1e-5 || d1 < 1e-5) ? 1e-6 : 0.01 * d0 / d1;
+    ha = fmin(ha, interval);
+#pragma unroll
+    for (int c = 0; c < NI; c++) {
+        q1[c] = fma(ha * dir, s.p[c], s.q[c]);
+        p1[c] = fma(ha * dir, F0[c], s.p[c]);
+    }
+    s.force(q1, F1);
+    double s2 = 0.0;
+#pragma unroll
+    for (int c = 0; c < NI; c++) {
+        const double iq = 1.0 / fma(fabs(s.q[c]), rtol, atol), ip = 1.0 / fma(fabs(s.p[c]), rtol, atol);
+        const double dq = (p1[c] - s.p[c]) * iq, dp = (F1[c] - F0[c]) * ip;
+        if (on[c]) s2 += dq * dq + dp * dp;
+    }
+    const double d2 = sqrt(tile_sum<L>(s2) / D) / ha;
+    double hb;
+    if (d1 <= 1e-15 && d2 <= 1e-15) hb = fmax(1e-6, 1e-3 * ha);
+    else hb = root8(0.01 / fmax(d1, d2));
+    return fmin(fmin(100.0 * ha, hb), interval);
+}
 
 // functors handed to dop8_stages (plain structs: generic lambdas with array-reference
 // parameters of dependent extent crash cudafe++ 12.9)
@@ -387,11 +405,11 @@ struct LdHook {
 };
 
 // ---- the run kernel: fixed or adaptive, with renormalisation / indicator ----------------------
-template <class Sys, int K, int L, int MODE, int IND, bool ADAPT, int TPB, int MINB>
+// S = the per-lane state class of a layout (Col<Sys,K,L> here, Chain<NP,K> in chain_kernels.cuh)
+template <class C, int MODE, int IND, bool ADAPT, int TPB, int MINB>
 __global__ void __launch_bounds__(TPB, MINB)
-col_run_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, const RunArgs a) {
-    using C = Col<Sys, K, L>;
-    constexpr int NI = C::NI;
+run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const RunArgs a) {
+    constexpr int NI = C::NI, L = C::L, K = C::K;
     const long long gt = (long long)blockIdx.x * TPB + threadIdx.x;
     const long long traj = gt / L;
     const bool valid = traj < a.n_ic;
@@ -444,7 +462,7 @@ col_run_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, 
         t = a.t0 + (double)a.n_steps * a.h;
     } else {
         const double dir = (a.t_end >= a.t0) ? 1.0 : -1.0;
-        double h_abs = a.h0 > 0.0 ? a.h0 : s.initial_step(fabs(a.t_end - a.t0), dir, a.rtol, a.atol);
+        double h_abs = a.h0 > 0.0 ? a.h0 : initial_step(s, fabs(a.t_end - a.t0), dir, a.rtol, a.atol);
         long long attempts = 0;
         bool rejected = false;
         double min_step = 0.0;
@@ -524,17 +542,7 @@ col_run_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, 
     if constexpr (IND != IND_NONE) ind = s.template indicator<IND>();
     if (!valid) return;
     s.store(a.y, a.w, a.n_ic, ic, bad);
-    if constexpr (K > 0) {
-        const double elapsed = t - a.t0;
-#pragma unroll
-        for (int j = 0; j < C::CPL; j++) {
-            if (s.is_dev(j)) {
-                const long long o = (long long)(s.col_of(j) - 1) * a.n_ic + ic;
-                if (a.logacc) a.logacc[o] = bad ? nan("") : a.logacc[o] + s.lg[j];
-                if (a.lambda) a.lambda[o] = (bad || elapsed == 0.0) ? nan("") : s.lg[j] / elapsed;
-            }
-        }
-    }
+    if constexpr (K > 0) s.store_logs(a, ic, bad, t - a.t0);
     if (s.lt == 0) {
         if constexpr (IND != IND_NONE) {
             if (a.series) {
