@@ -30,7 +30,7 @@ sys.path.insert(0, ROOT)
 METRIC = "trajectory RK-steps/sec (FP64, incl. variational eqs)"
 UNIT = "RK-steps/s"
 # algorithmic FP64 flop per RK-step of the formulation that runs
-FLOP_PER_STEP = {"C2": 640.0, "C1sat": 1128.0}
+FLOP_PER_STEP = {"C2": 640.0, "C1sat": 1216.0}
 NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12  # 37.2
 
 
@@ -103,6 +103,23 @@ def workload_inputs(args, rank, world):
     return dict(y0=y0, w0=w0, h=0.01, n_steps=2000, rk_steps=1.0 * y0.shape[1] * 2000)
 
 
+def oracle_sample(orc, args, target_s):
+    """A sub-grid of the C2 grid (every k-th row and column, full horizon) sized from a short
+    calibration run so that the oracle, as it stands, needs about target_s seconds on it."""
+    from paper_2507_00622_b200 import workloads as W
+    cores = orc.default_threads()
+    yc = W.hh_grid(0.125, 64, 64)
+    orc.ld(0, None, yc[:, :64].copy(), 0.0, 0.01, 10, precision="f64", threads=cores)  # thread start-up
+    t = time.perf_counter()
+    orc.ld(0, None, yc, 0.0, 0.01, 300, precision="f64", threads=cores)
+    rate = 2.0 * 4096 * 300 / (time.perf_counter() - t)
+    sub = int(np.sqrt(max(rate * target_s / (2.0 * args.n_steps), 256.0)))
+    sub = max(16, min(sub, args.side))
+    idx = np.unique(np.linspace(0, args.side - 1, sub).round().astype(int))
+    rows = [W.hh_grid(0.125, args.side, args.side, i_range=(int(i), int(i) + 1))[:, idx] for i in idx]
+    return np.ascontiguousarray(np.concatenate(rows, axis=1)), len(idx), cores
+
+
 def run_reference(args):
     """The CPU oracle, as it stands, on a bounded sample of the same workload."""
     rank = int(os.environ.get("RANK", "0"))
@@ -111,11 +128,7 @@ def run_reference(args):
     from oracle import chaos_oracle as orc
     from paper_2507_00622_b200 import workloads as W
     orc.build()
-    cores = orc.default_threads()
-    sub = 48  # 48 x 48 sub-grid of the 1024 x 1024 grid (every ~21st row / column), full horizon
-    idx = (np.arange(sub) * (args.side // sub))
-    full_rows = [W.hh_grid(0.125, args.side, args.side, i_range=(int(i), int(i) + 1))[:, idx] for i in idx]
-    y0 = np.ascontiguousarray(np.concatenate(full_rows, axis=1))
+    y0, sub, cores = oracle_sample(orc, args, target_s=120.0 / max(1, args.steps + args.warmup))
     n_steps = args.n_steps
     times = []
     for it in range(args.warmup + args.steps):
@@ -294,10 +307,7 @@ def main():
     if not args.no_cpu_baseline and world == 1 and args.workload == "C2":
         from oracle import chaos_oracle as orc
         orc.build()
-        cores = orc.default_threads()
-        sub = 48
-        idx = np.arange(sub) * (args.side // sub)
-        ys = np.ascontiguousarray(wl["y0"].reshape(4, args.side, args.side)[:, idx][:, :, idx].reshape(4, -1))
+        ys, sub, cores = oracle_sample(orc, args, target_s=15.0)
         t0 = time.perf_counter()
         orc.ld(0, None, ys, 0.0, 0.01, wl["n_steps"], precision="f64", threads=cores)
         dt = time.perf_counter() - t0

@@ -21,6 +21,7 @@ struct Chain {
     static constexpr int NI = NCOL;
     static constexpr int N = 2 * NP;
     static constexpr int D = N * NCOL;
+    static constexpr int NCOMP = 1;  // item 0: the orbit coordinate -- compensated update
     using Params = FputParams;
 
     Params prm;

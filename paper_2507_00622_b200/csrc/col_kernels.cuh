@@ -101,6 +101,7 @@ struct Col {
     static constexpr int CPL = (NCOL + L - 1) / L;
     static constexpr int NI = CPL * ND;
     static constexpr int D = N * NCOL;
+    static constexpr int NCOMP = ND;  // item j = 0: the orbit (lane 0) -- compensated update
     using Params = typename Sys::Params;
 
     Params prm;
@@ -428,6 +429,10 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
     int status = ST_OK;
     double t = a.t0;
     long long slot = 0;
+    constexpr int NC = C::NCOMP > 0 ? C::NCOMP : 1;
+    double qc[NC], pc[NC], qcn[NC], pcn[NC];  // carried rounding errors of the orbit update
+#pragma unroll
+    for (int c = 0; c < NC; c++) qc[c] = pc[c] = 0.0;
 
     if constexpr (!ADAPT) {
         int cd = a.m, sd = a.sample_every;
@@ -435,11 +440,16 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
             double F[12][NI];
             dop8_stages<NI, true>(tab, 0.0, 0.0, s.q, s.p, F, force, nohook);
             double qn[NI], pn[NI];
-            dop8_solution<NI, true>(tab, 0.0, 0.0, s.q, s.p, F, qn, pn);
+            dop8_solution<NI, C::NCOMP, true>(tab, 0.0, 0.0, s.q, s.p, F, qn, pn, qc, pc, qcn, pcn);
 #pragma unroll
             for (int c = 0; c < NI; c++) {
                 s.q[c] = qn[c];
                 s.p[c] = pn[c];
+            }
+#pragma unroll
+            for (int c = 0; c < NC; c++) {
+                qc[c] = qcn[c];
+                pc[c] = pcn[c];
             }
             if constexpr (MODE != MODE_NONE) {
                 if (--cd == 0 || st == a.n_steps) {
@@ -493,7 +503,7 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
             double F[12][NI];
             dop8_stages<NI, false>(tab, h, h * h, s.q, s.p, F, force, nohook);
             double qn[NI], pn[NI];
-            dop8_solution<NI, false>(tab, h, h * h, s.q, s.p, F, qn, pn);
+            dop8_solution<NI, C::NCOMP, false>(tab, h, h * h, s.q, s.p, F, qn, pn, qc, pc, qcn, pcn);
             double S5, S3;
             dop8_error_sums<NI>(tab, h, s.q, s.p, qn, pn, F, a.rtol, a.atol, on, S5, S3);
             S5 = tile_sum<L>(S5);
@@ -511,6 +521,11 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
                     for (int c = 0; c < NI; c++) {
                         s.q[c] = qn[c];
                         s.p[c] = pn[c];
+                    }
+#pragma unroll
+                    for (int c = 0; c < NC; c++) {
+                        qc[c] = qcn[c];
+                        pc[c] = pcn[c];
                     }
                     n_acc++;
                     rejected = false;
@@ -584,7 +599,8 @@ col_ld_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, c
         double F[12][NI];
         dop8_stages<NI, true>(tab, 0.0, 0.0, s.q, s.p, F, force, hook);
         double qn[NI], pn[NI];
-        dop8_solution<NI, true>(tab, 0.0, 0.0, s.q, s.p, F, qn, pn);
+        double z[1] = {0.0}, zn[1];
+        dop8_solution<NI, 0, true>(tab, 0.0, 0.0, s.q, s.p, F, qn, pn, z, z, zn, zn);
 #pragma unroll
         for (int c = 0; c < NI; c++) {
             s.q[c] = qn[c];

@@ -107,23 +107,30 @@ __device__ __forceinline__ void dop8_stages(const Tab& tab, double h, double h2,
     });
 }
 
-// 8th-order solution from the stage forces
-template <int NI, bool PREMUL>
+// 8th-order solution from the stage forces.  The first NCOMP items (the orbit's) are advanced
+// with a compensated sum: y+ = y + (dy + c) by Fast2Sum, the rounding
+// error of that one addition -- which is ~1/h times larger than every other rounding error of a
+// step -- is carried in c to the next step.  qc/pc: carried words in, qcn/pcn: out.
+template <int NI, int NCOMP, bool PREMUL>
 __device__ __forceinline__ void dop8_solution(const Tab& tab, double h, double h2, const double (&q)[NI],
                                               const double (&p)[NI], const double (&F)[12][NI],
-                                              double (&qn)[NI], double (&pn)[NI]) {
+                                              double (&qn)[NI], double (&pn)[NI],
+                                              const double (&qc)[NCOMP > 0 ? NCOMP : 1],
+                                              const double (&pc)[NCOMP > 0 ? NCOMP : 1],
+                                              double (&qcn)[NCOMP > 0 ? NCOMP : 1],
+                                              double (&pcn)[NCOMP > 0 ? NCOMP : 1]) {
 #pragma unroll
     for (int c = 0; c < NI; c++) {
+        const bool comp = c < NCOMP;
+        double aq, ap;
         if constexpr (PREMUL) {
-            double aq = fma(tab.h, p[c], q[c]);
-            double ap = p[c];
+            aq = comp ? fma(tab.h, p[c], qc[comp ? c : 0]) : fma(tab.h, p[c], q[c]);
+            ap = comp ? pc[comp ? c : 0] : p[c];
             static_for<0, 12>([&](auto lc) {
                 constexpr int l = decltype(lc)::value;
                 if constexpr (coef::BQ[l] != 0.0) aq = fma(tab.bq[l], F[l][c], aq);
                 if constexpr (coef::B[l] != 0.0) ap = fma(tab.bp[l], F[l][c], ap);
             });
-            qn[c] = aq;
-            pn[c] = ap;
         } else {
             double sq = tab.bq[0] * F[0][c];
             double sp = tab.bp[0] * F[0][c];
@@ -132,8 +139,18 @@ __device__ __forceinline__ void dop8_solution(const Tab& tab, double h, double h
                 if constexpr (coef::BQ[l] != 0.0) sq = fma(tab.bq[l], F[l][c], sq);
                 if constexpr (coef::B[l] != 0.0) sp = fma(tab.bp[l], F[l][c], sp);
             });
-            qn[c] = fma(h2, sq, fma(h, p[c], q[c]));
-            pn[c] = fma(h, sp, p[c]);
+            aq = comp ? fma(h2, sq, fma(h, p[c], qc[comp ? c : 0])) : fma(h2, sq, fma(h, p[c], q[c]));
+            ap = comp ? fma(h, sp, pc[comp ? c : 0]) : fma(h, sp, p[c]);
+        }
+        if (comp) {  // aq, ap are increments (+ carried error): Fast2Sum
+            const double tq = q[c] + aq, tp = p[c] + ap;
+            qcn[comp ? c : 0] = aq - (tq - q[c]);
+            pcn[comp ? c : 0] = ap - (tp - p[c]);
+            qn[c] = tq;
+            pn[c] = tp;
+        } else {
+            qn[c] = aq;
+            pn[c] = ap;
         }
     }
 }
