@@ -30,7 +30,13 @@ sys.path.insert(0, ROOT)
 METRIC = "trajectory RK-steps/sec (FP64, incl. variational eqs)"
 UNIT = "RK-steps/s"
 # algorithmic FP64 flop per RK-step of the formulation that runs
-FLOP_PER_STEP = {"C2": 640.0, "C1sat": 1216.0}
+FLOP_PER_STEP = {"C2": 640.0, "C1sat": 1216.0, "C3": 1812.0, "C4": 4213.0, "C5": 8492.0}
+WORKLOAD_LABEL = {
+    "C1sat": "C1sat: Henon-Heiles fixed-step SALI kernel of configs[0] on a saturating 512x512 ensemble, 2000 steps",
+    "C3": "C3: Henon-Heiles adaptive DOP8(5) rtol=atol=1e-12, 512x512 grid at E=1/6, t=1000, SALI (RK-step = attempted step)",
+    "C4": "C4: 3-DoF coupled oscillators, 65536 ICs, full Lyapunov spectrum (6 vectors, MGS every 10 steps), h=0.01, 1e5 steps",
+    "C5": "C5: FPUT-beta N=8, 65536 ICs, GALI_4 (renormalised every 10 steps), h=0.05, 2e4 steps",
+}
 NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12  # 37.2
 
 
@@ -40,7 +46,8 @@ def parse():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C2", choices=["C2", "C1sat"])
+    ap.add_argument("--workload", default="C2", choices=["C2", "C1sat", "C3", "C4", "C5"])
+    ap.add_argument("--shrink", type=int, default=1, help="C3/C4/C5: divide ensemble and horizon (profiling runs)")
     ap.add_argument("--side", type=int, default=1024, help="grid side per rank (C2)")
     ap.add_argument("--n-steps", type=int, default=5000, help="DOP8 steps per direction (C2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -152,6 +159,81 @@ def run_reference(args):
     }))
 
 
+def make_workload(chs, torch, args, rank, world):
+    """Device-resident inputs + the two step closures (device pointers / host buffers) of a workload."""
+    from paper_2507_00622_b200 import workloads as W
+    HH = chs.SYS_HENON_HEILES
+    name = args.workload
+    if name in ("C2", "C1sat"):
+        wl = workload_inputs(args, rank, world)
+        y0_host = torch.from_numpy(wl["y0"]).pin_memory()
+        y0 = y0_host.cuda()
+        n_ic = y0.shape[1]
+    if name == "C2":
+        f = torch.empty(n_ic, dtype=torch.float64, device="cuda")
+        b = torch.empty(n_ic, dtype=torch.float64, device="cuda")
+        f_host = torch.empty(n_ic, dtype=torch.float64).pin_memory()
+        b_host = torch.empty(n_ic, dtype=torch.float64).pin_memory()
+        return dict(wl=wl, n_ic=n_ic, h2d=y0_host.numel() * 8, d2h=2 * n_ic * 8,
+                    kinfo=chs.kernel_info(HH, None, chs.WHAT_LD, n_ic=n_ic),
+                    step_dev=lambda: chs.ld(HH, None, y0, 0.0, wl["h"], wl["n_steps"], out_fwd=f, out_bwd=b),
+                    step_e2e=lambda: chs.ld_host(HH, None, y0_host, 0.0, wl["h"], wl["n_steps"], f_host, b_host))
+    # the other workloads advance y, w in place: every step starts from a fresh device copy made
+    # OUTSIDE the timed events (prepare), so only the library's kernel is timed
+    if name == "C1sat":
+        sysid, prm, w0_np, k = HH, None, wl["w0"], 2
+        call = lambda y, w: chs.sali(HH, None, y, w, renorm_every=1, h=wl["h"], n_steps=wl["n_steps"])
+        host = lambda y, w, o: chs.sali_host(HH, None, y, w, o, renorm_every=1, h=wl["h"], n_steps=wl["n_steps"])
+        out_rows, what, adaptive = 1, chs.WHAT_SALI, False
+    else:
+        n_full = {"C3": 512 * 512, "C4": 65536, "C5": 65536}[name]
+        cfg = W.config(name, n_ic=max(1024, n_full // args.shrink) if args.shrink > 1 else None)
+        sysid, prm, w0_np = cfg["system"], cfg["params"], cfg["w"]
+        k = w0_np.shape[0]
+        y0_host = torch.from_numpy(cfg["y"]).pin_memory()
+        y0 = y0_host.cuda()
+        n_ic = y0.shape[1]
+        ns = max(10, cfg.get("n_steps", 0) // args.shrink)
+        if name == "C3":
+            t_end = cfg["t_end"] / args.shrink
+            rep = chs.Report(n_ic, "cuda")
+            call = lambda y, w: chs.sali(sysid, prm, y, w, renorm_every=1, adaptive=True, t_end=t_end, rtol=1e-12,
+                                         atol=1e-12, report=rep)
+            host = lambda y, w, o: chs.sali_host(sysid, prm, y, w, o, renorm_every=1, adaptive=True, t_end=t_end,
+                                                 rtol=1e-12, atol=1e-12)
+            out_rows, what, adaptive = 1, chs.WHAT_SALI, True
+            wl = dict(rk_steps=None, report=rep)
+        elif name == "C4":
+            call = lambda y, w: chs.lyap(sysid, prm, y, w, renorm_every=10, h=cfg["h"], n_steps=ns)
+            host = lambda y, w, o: chs.lyap_host(sysid, prm, y, w, o, renorm_every=10, h=cfg["h"], n_steps=ns)
+            out_rows, what, adaptive = k, chs.WHAT_LYAP, False
+            wl = dict(rk_steps=1.0 * n_ic * ns)
+        else:
+            call = lambda y, w: chs.gali(sysid, prm, y, w, renorm_every=10, h=cfg["h"], n_steps=ns)
+            host = lambda y, w, o: chs.gali_host(sysid, prm, y, w, o, renorm_every=10, h=cfg["h"], n_steps=ns)
+            out_rows, what, adaptive = 1, chs.WHAT_GALI, False
+            wl = dict(rk_steps=1.0 * n_ic * ns)
+    w0_host = torch.from_numpy(w0_np).pin_memory()
+    w0 = w0_host.cuda()
+    yb, wb = torch.empty_like(y0), torch.empty_like(w0)
+    yh, wh = torch.empty_like(y0_host).pin_memory(), torch.empty_like(w0_host).pin_memory()
+    oh = torch.empty((out_rows, n_ic), dtype=torch.float64).pin_memory()
+
+    def prepare():
+        yb.copy_(y0)
+        wb.copy_(w0)
+
+    def step_e2e():
+        yh.copy_(y0_host)
+        wh.copy_(w0_host)
+        host(yh, wh, oh)
+
+    return dict(wl=wl, n_ic=n_ic, h2d=(y0_host.numel() + w0_host.numel()) * 8,
+                d2h=(y0_host.numel() + w0_host.numel() + out_rows * n_ic) * 8,
+                kinfo=chs.kernel_info(sysid, prm, what, k=k, adaptive=adaptive, n_ic=n_ic),
+                step_dev=lambda: call(yb, wb), step_e2e=step_e2e, prepare=prepare)
+
+
 def main():
     args = parse()
     if args.impl == "reference":
@@ -175,54 +257,19 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    wl = workload_inputs(args, rank, world)
-    y0_host = torch.from_numpy(wl["y0"]).pin_memory()
-    y0 = y0_host.cuda()
-    n_ic = y0.shape[1]
-    HH = chs.SYS_HENON_HEILES
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
-
-    if args.workload == "C2":
-        f = torch.empty(n_ic, dtype=torch.float64, device="cuda")
-        b = torch.empty(n_ic, dtype=torch.float64, device="cuda")
-        f_host = torch.empty(n_ic, dtype=torch.float64).pin_memory()
-        b_host = torch.empty(n_ic, dtype=torch.float64).pin_memory()
-
-        def step_dev():
-            chs.ld(HH, None, y0, 0.0, wl["h"], wl["n_steps"], out_fwd=f, out_bwd=b)
-
-        def step_e2e():
-            chs.ld_host(HH, None, y0_host, 0.0, wl["h"], wl["n_steps"], f_host, b_host)
-
-        h2d, d2h = y0_host.numel() * 8, 2 * n_ic * 8
-        kinfo = chs.kernel_info(HH, None, chs.WHAT_LD, n_ic=n_ic)
-        launches_per_step = 1
-    else:
-        w0_host = torch.from_numpy(wl["w0"]).pin_memory()
-        w0 = w0_host.cuda()
-        yb, wb = torch.empty_like(y0), torch.empty_like(w0)
-        yh, wh = torch.empty_like(y0_host).pin_memory(), torch.empty_like(w0_host).pin_memory()
-        sh = torch.empty((1, n_ic), dtype=torch.float64).pin_memory()
-
-        def step_dev():
-            yb.copy_(y0)
-            wb.copy_(w0)
-            chs.sali(HH, None, yb, wb, renorm_every=1, h=wl["h"], n_steps=wl["n_steps"])
-
-        def step_e2e():
-            yh.copy_(y0_host)
-            wh.copy_(w0_host)
-            chs.sali_host(HH, None, yh, wh, sh, renorm_every=1, h=wl["h"], n_steps=wl["n_steps"])
-
-        h2d, d2h = (y0_host.numel() + w0_host.numel()) * 8, (y0_host.numel() + w0_host.numel() + n_ic) * 8
-        kinfo = chs.kernel_info(HH, None, chs.WHAT_SALI, k=2, n_ic=n_ic)
-        launches_per_step = 1
+    wk = make_workload(chs, torch, args, rank, world)
+    wl, step_dev, step_e2e, h2d, d2h, kinfo = wk["wl"], wk["step_dev"], wk["step_e2e"], wk["h2d"], wk["d2h"], wk["kinfo"]
+    n_ic = wk["n_ic"]
+    launches_per_step = 1
 
     def timed(fn, n):
         """n iterations, each bracketed by CUDA events on the launching stream, L2 flushed between."""
         ms = []
         for _ in range(n):
             flush.fill_(1)
+            if "prepare" in wk:
+                wk["prepare"]()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             torch.cuda.synchronize()
             e0.record()
@@ -243,6 +290,8 @@ def main():
     dfma_tflops = probe_flop / (pe0.elapsed_time(pe1) * 1e-3) / 1e12
 
     for _ in range(max(args.warmup, 0)):
+        if "prepare" in wk:
+            wk["prepare"]()
         step_dev()
     barrier()
     with ClockSampler(local) as cs:
@@ -256,6 +305,10 @@ def main():
         tt = torch.tensor([t_dev], dtype=torch.float64, device="cuda")
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
         t_dev = tt.item()
+    if wl["rk_steps"] is None:   # adaptive: one RK-step = one ATTEMPTED step (accepted + rejected), counted by the kernel
+        rp = wl["report"]
+        wl["rk_steps"] = float((rp.n_accepted.sum() + rp.n_rejected.sum()).item())
+        wl["accepted"], wl["rejected"] = int(rp.n_accepted.sum().item()), int(rp.n_rejected.sum().item())
     value = wl["rk_steps"] * world * args.steps / t_dev
 
     # end to end: host buffers through the C ABI's host entry point, copies inside the timed region
@@ -286,8 +339,7 @@ def main():
         "config": {
             "workload": ("C2: Henon-Heiles Lagrangian descriptor (arc length), E=1/8, %dx%d grid per GPU, "
                          "fixed DOP8 h=0.01, %d steps forward + %d backward" % (args.side, args.side, wl["n_steps"], wl["n_steps"]))
-            if args.workload == "C2" else
-            "C1sat: Henon-Heiles fixed-step SALI kernel of configs[0] on a saturating 512x512 ensemble, 2000 steps",
+            if args.workload == "C2" else WORKLOAD_LABEL[args.workload] + (" (shrink %d)" % args.shrink if args.shrink > 1 else ""),
             "n_ic_per_gpu": int(n_ic), "rk_steps_per_step": wl["rk_steps"] * world,
             "l2": "flushed between timed iterations (256 MiB write)",
             "kernel": kinfo,

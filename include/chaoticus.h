@@ -148,6 +148,10 @@ int chaoticus_integrate_host(const chs_problem* pb, long long n_ic, double* y, c
  * n_blocks x n_threads threads x iters x 16 DFMA each; out DEVICE [n_blocks*n_threads]
  * (keeps the work alive).  Used by bench.py to measure the FP64 FMA peak of the device. */
 int chaoticus_dfma_probe(long long iters, int n_blocks, int n_threads, double* out, void* stream);
+/* Variants of the probe: mode 0 as above (fixed register operands); mode 1: the multiplier comes
+ * from the constant bank, as the step kernels read the tableau; mode 2: three distinct register
+ * operands per DFMA (register-file bandwidth included). */
+int chaoticus_dfma_probe_mode(int mode, long long iters, int n_blocks, int n_threads, double* out, void* stream);
 
 /* Kernel launch shape the library would use for a call (for reporting): writes threads per
  * block, blocks, lanes per trajectory, registers per thread, spill bytes.  what: 0 integrate,

@@ -24,7 +24,8 @@ EXPORTS = [
     "chaoticus_version", "chaoticus_last_error", "chaoticus_dim", "chaoticus_n_samples",
     "chaoticus_integrate_fixed", "chaoticus_integrate_adaptive", "chaoticus_sali", "chaoticus_gali",
     "chaoticus_ld", "chaoticus_lyap", "chaoticus_ld_host", "chaoticus_sali_host", "chaoticus_gali_host",
-    "chaoticus_lyap_host", "chaoticus_integrate_host", "chaoticus_dfma_probe", "chaoticus_kernel_info",
+    "chaoticus_lyap_host", "chaoticus_integrate_host", "chaoticus_dfma_probe", "chaoticus_dfma_probe_mode",
+    "chaoticus_kernel_info",
 ]
 
 
@@ -70,6 +71,7 @@ def _load():
     lib.chaoticus_lyap_host.argtypes = [PP, ll, vp, vp, i, SP, i, vp, vp, RP]
     lib.chaoticus_integrate_host.argtypes = [PP, ll, vp, SP, RP]
     lib.chaoticus_dfma_probe.argtypes = [ll, i, i, vp, vp]
+    lib.chaoticus_dfma_probe_mode.argtypes = [i, ll, i, i, vp, vp]
     lib.chaoticus_kernel_info.argtypes = [PP, i, i, i, ll, C.POINTER(C.c_int)]
     return lib
 
@@ -272,10 +274,10 @@ def integrate_host(system, params, y, **stepper):
 
 
 # ---- measurement aids --------------------------------------------------------------------------
-def dfma_probe(iters, n_blocks, n_threads=256):
+def dfma_probe(iters, n_blocks, n_threads=256, mode=0):
     """Launches the DFMA peak probe on the current stream; returns the FP64 flop it performs."""
     out = torch.empty(n_blocks * n_threads, dtype=torch.float64, device="cuda")
-    _check(_lib.chaoticus_dfma_probe(int(iters), n_blocks, n_threads, out.data_ptr(), _stream()))
+    _check(_lib.chaoticus_dfma_probe_mode(mode, int(iters), n_blocks, n_threads, out.data_ptr(), _stream()))
     return 2.0 * 16.0 * iters * n_blocks * n_threads, out
 
 
