@@ -70,6 +70,12 @@ int dispatch(const chs::LaunchReq& rq) {
     if ((r = chs::try_launch_c3(rq)) != -1) return r;
     if ((r = chs::try_launch_c3_lyap(rq)) != -1) return r;
     if ((r = chs::try_launch_fput(rq)) != -1) return r;
+    if ((r = chs::try_launch_fput_adapt(rq)) != -1) return r;
+    if ((r = chs::try_launch_fput_n4(rq)) != -1) return r;
+    if ((r = chs::try_launch_fput_n16(rq)) != -1) return r;
+    if ((r = chs::try_launch_fput_n32(rq)) != -1) return r;
+    if ((r = chs::try_launch_hh_adapt2(rq)) != -1) return r;
+    if ((r = chs::try_launch_c3_more(rq)) != -1) return r;
     return -1;
 }
 

@@ -400,7 +400,7 @@ struct LdHook {
                 });
                 n2 = fma(P, P, fma(F[i][c], F[i][c], n2));
             }
-            M = fma(tab.bl[i], sqrt(n2), M);
+            M = fma(tab.bl[i], sqrt(tile_sum<C::L>(n2)), M);
         }
     }
 };
@@ -579,16 +579,19 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
 // with +h give mirror-image states bit for bit and the same |f|.
 // M += |h| sum_i b_i |k_i|_2 with k_i = (P_i, F_i) the stage derivative; P_i is formed only at
 // the 8 stages with b_i != 0.
-template <class Sys, int TPB, int MINB>
+// C = a layout with K = 0 (Col<Sys,0,1>: one thread per (direction, IC); Chain<N,0>: one tile).
+template <class C, int TPB, int MINB>
 __global__ void __launch_bounds__(TPB, MINB)
-col_ld_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, const RunArgs a, int dir_first,
-              int n_dirs) {
-    using C = Col<Sys, 0, 1>;
-    constexpr int NI = C::NI;
+ld_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const RunArgs a, int dir_first,
+          int n_dirs) {
+    constexpr int NI = C::NI, L = C::L;
     const long long gt = (long long)blockIdx.x * TPB + threadIdx.x;
-    if (gt >= a.n_ic * n_dirs) return;
-    const int dsel = dir_first + (int)(gt / a.n_ic);  // 0 forward, 1 backward
-    const long long ic = gt % a.n_ic;
+    const long long task = gt / L, n_task = a.n_ic * n_dirs;
+    const bool valid = task < n_task;
+    if (L == 1 && !valid) return;
+    const long long tk = valid ? task : n_task - 1;  // padding tiles shadow the last task (shuffles stay convergent)
+    const int dsel = dir_first + (int)(tk / a.n_ic);  // 0 forward, 1 backward
+    const long long ic = tk % a.n_ic;
     C s;
     s.init(prm);
     s.load(a.y0, nullptr, a.n_ic, ic, dsel == 0 ? 1.0 : -1.0);
@@ -609,7 +612,7 @@ col_ld_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, c
     }
     const bool ok = s.finite_all();
     double* out = dsel == 0 ? a.ld_fwd : a.ld_bwd;
-    out[ic] = ok ? M : nan("");
+    if (valid && s.lt == 0) out[ic] = ok ? M : nan("");
 }
 
 }  // namespace chs

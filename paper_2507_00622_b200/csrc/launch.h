@@ -32,6 +32,12 @@ int try_launch_hh_adapt(const LaunchReq& rq);
 int try_launch_c3(const LaunchReq& rq);
 int try_launch_c3_lyap(const LaunchReq& rq);
 int try_launch_fput(const LaunchReq& rq);
+int try_launch_fput_adapt(const LaunchReq& rq);
+int try_launch_fput_n4(const LaunchReq& rq);
+int try_launch_fput_n16(const LaunchReq& rq);
+int try_launch_fput_n32(const LaunchReq& rq);
+int try_launch_hh_adapt2(const LaunchReq& rq);
+int try_launch_c3_more(const LaunchReq& rq);
 
 template <class Kern>
 inline int finish_launch(const LaunchReq& rq, Kern kern, int tpb, int lanes, long long n_threads) {
@@ -64,7 +70,7 @@ template <class Sys, int TPB, int MINB>
 inline int run_ld(const LaunchReq& rq) {
     typename Sys::Params prm;
     if (!Sys::make_params(rq.params, rq.n_params, prm)) return (int)cudaErrorInvalidValue;
-    auto kern = col_ld_kernel<Sys, TPB, MINB>;
+    auto kern = ld_kernel<Col<Sys, 0, 1>, TPB, MINB>;
     const long long n_threads = rq.args.n_ic * rq.n_dirs;
     int r = finish_launch(rq, kern, TPB, 1, n_threads);
     if (r != -2) return r;

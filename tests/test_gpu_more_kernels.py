@@ -1,0 +1,168 @@
+"""GPU parity for the wider kernel set (SURVEY.md section 8f "next" rows): other chain lengths
+of the FPUT chain layout (N = 4, 16, 32; a full warp per trajectory at N = 32), the LD on the
+chain layout, adaptive Lyapunov / GALI, and the remaining k of the 3-DoF system."""
+import numpy as np
+import pytest
+
+from paper_2507_00622_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+HH, C3, FPUT = W.SYS_HENON_HEILES, W.SYS_COUPLED3, W.SYS_FPUT
+
+
+@pytest.fixture(scope="module")
+def chs():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2507_00622_b200 import binding
+    return binding
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def rel_state(a, b):
+    return np.linalg.norm(a - b, axis=0) / np.linalg.norm(b, axis=0)
+
+
+def lam_err(lam, ref, T):
+    return (np.abs(lam - ref) / np.maximum(np.abs(ref).max(0), 1.0 / T)).max()
+
+
+@pytest.mark.parametrize("N", [4, 16, 32])
+def test_fput_other_lengths(chs, orc, N):
+    n_ic = 45          # ragged: 45 tiles of N lanes
+    prm = W.fput_params(N, 1.0, 0.1, 0.8)
+    y0 = W.fput_ics(n_ic, N, seed=3 + N, E=0.1 * N)
+    w0 = W.deviation_vectors(n_ic, 4, 2 * N, 50 + N, "orthonormal")
+    # plain integration
+    yo = y0.copy()
+    orc.integrate_fixed(FPUT, prm, yo, 0.0, 0.05, 1000, precision="f80")
+    yg = dev(y0)
+    chs.integrate_fixed(FPUT, prm, yg, 0.0, 0.05, 1000)
+    assert rel_state(yg.cpu().numpy(), yo).max() <= 1e-10
+    # GALI_4, fixed step
+    yo, wo = y0.copy(), w0.copy()
+    go = orc.gali(FPUT, prm, yo, wo, renorm_every=10, sample_every=10, h=0.05, n_steps=1000, precision="f80")["series"]
+    yg, wg = dev(y0), dev(w0)
+    gg = chs.gali(FPUT, prm, yg, wg, renorm_every=10, sample_every=10, h=0.05, n_steps=1000).cpu().numpy()
+    assert go.min() > 1e-9 and np.abs(gg / go - 1).max() <= 1e-8
+    assert np.abs(wg.cpu().numpy() - wo).max() <= 1e-9
+    # Lyapunov k = 4 and SALI
+    yo, wo = y0.copy(), w0.copy()
+    lo = orc.lyap(FPUT, prm, yo, wo, renorm_every=10, h=0.05, n_steps=1000, precision="f80")["lam"]
+    lg = chs.lyap(FPUT, prm, dev(y0), dev(w0), renorm_every=10, h=0.05, n_steps=1000).cpu().numpy()
+    assert lam_err(lg, lo, 50.0) <= 1e-8
+    w2 = np.ascontiguousarray(w0[:2])
+    so = orc.sali(FPUT, prm, y0.copy(), w2.copy(), renorm_every=5, h=0.05, n_steps=600, precision="f80")["series"]
+    sg = chs.sali(FPUT, prm, dev(y0), dev(w2), renorm_every=5, h=0.05, n_steps=600).cpu().numpy()
+    assert np.abs(sg / so - 1).max() <= 1e-8
+    # LD on the chain layout (tile-wide norm by shuffles), both directions
+    fo, bo = orc.ld(FPUT, prm, y0, 0.0, 0.05, 400, precision="f80")
+    f, b = chs.ld(FPUT, prm, dev(y0), 0.0, 0.05, 400)
+    assert np.abs(f.cpu().numpy() / fo - 1).max() <= 1e-8 and np.abs(b.cpu().numpy() / bo - 1).max() <= 1e-8
+    # adaptive GALI_4 (the paper's Fig. 3 solver, atol = 1e-8: PAPER.md:129)
+    yo, wo = y0.copy(), w0.copy()
+    ro = orc.gali(FPUT, prm, yo, wo, renorm_every=1, adaptive=True, t_end=20.0, rtol=1e-8, atol=1e-8, precision="f80")
+    rep = chs.Report(n_ic, "cuda")
+    ga = chs.gali(FPUT, prm, dev(y0), dev(w0), renorm_every=1, adaptive=True, t_end=20.0, rtol=1e-8, atol=1e-8,
+                  report=rep).cpu().numpy()
+    assert (rep.status.cpu().numpy() == 0).all()
+    assert np.abs(ga / ro["series"] - 1).max() <= 1e-4
+    assert abs(rep.n_accepted.cpu().numpy().sum() / ro["n_accepted"].sum() - 1) <= 2e-2
+
+
+def test_fput8_ld_and_adaptive_set(chs, orc):
+    cfg = W.config("C5", n_ic=70)
+    y0, w0, prm = cfg["y"], cfg["w"], cfg["params"]
+    fo, bo = orc.ld(FPUT, prm, y0, 0.0, 0.05, 600, precision="f80")
+    f, b = chs.ld(FPUT, prm, dev(y0), 0.0, 0.05, 600)
+    assert np.abs(f.cpu().numpy() / fo - 1).max() <= 1e-8 and np.abs(b.cpu().numpy() / bo - 1).max() <= 1e-8
+    st = dict(adaptive=True, t_end=30.0, rtol=1e-9, atol=1e-9)
+    for k in (1, 4):
+        wk = np.ascontiguousarray(w0[:k])
+        lo = orc.lyap(FPUT, prm, y0.copy(), wk.copy(), renorm_every=3, precision="f80", **st)["lam"]
+        lg = chs.lyap(FPUT, prm, dev(y0), dev(wk), renorm_every=3, **st).cpu().numpy()
+        assert lam_err(lg, lo, 30.0) <= 1e-5
+    for k in (2, 3):
+        wk = np.ascontiguousarray(w0[:k])
+        go = orc.gali(FPUT, prm, y0.copy(), wk.copy(), renorm_every=2, precision="f80", **st)["series"]
+        gg = chs.gali(FPUT, prm, dev(y0), dev(wk), renorm_every=2, **st).cpu().numpy()
+        assert np.abs(gg / go - 1).max() <= 1e-5
+    w2 = np.ascontiguousarray(w0[:2])
+    so = orc.sali(FPUT, prm, y0.copy(), w2.copy(), renorm_every=2, precision="f80", **st)["series"]
+    sg = chs.sali(FPUT, prm, dev(y0), dev(w2), renorm_every=2, **st).cpu().numpy()
+    assert np.abs(sg / so - 1).max() <= 1e-5
+    yo = y0.copy()
+    orc.integrate_adaptive(FPUT, prm, yo, 0.0, 30.0, 1e-11, 1e-11, precision="f80")
+    yg = dev(y0)
+    chs.integrate_adaptive(FPUT, prm, yg, 0.0, 30.0, 1e-11, 1e-11)
+    assert rel_state(yg.cpu().numpy(), yo).max() <= 1e-8
+
+
+@pytest.mark.parametrize("k", [3, 4])
+def test_hh_adaptive_gali_lyap(chs, orc, k):
+    y0 = W.hh_grid(0.125, 9, 11)
+    n_ic = y0.shape[1]
+    w0 = W.deviation_vectors(n_ic, k, 4, 21, "orthonormal")
+    st = dict(adaptive=True, t_end=40.0, rtol=1e-11, atol=1e-11)
+    go = orc.gali(HH, None, y0.copy(), w0.copy(), renorm_every=1, precision="f80", **st)["series"]
+    gg = chs.gali(HH, None, dev(y0), dev(w0), renorm_every=1, **st).cpu().numpy()
+    big = go > 1e-10
+    assert np.abs(gg[big] / go[big] - 1).max() <= 1e-5 and np.abs(gg[~big] - go[~big]).max(initial=0) <= 1e-12
+    lo = orc.lyap(HH, None, y0.copy(), w0.copy(), renorm_every=2, precision="f80", **st)["lam"]
+    lg = chs.lyap(HH, None, dev(y0), dev(w0), renorm_every=2, **st).cpu().numpy()
+    assert lam_err(lg, lo, 40.0) <= 1e-6
+
+
+@pytest.mark.parametrize("k", [2, 3, 4, 5])
+def test_coupled3_lyap_other_k(chs, orc, k):
+    cfg = W.config("C4", n_ic=77)
+    y0, prm = cfg["y"], cfg["params"]
+    w0 = np.ascontiguousarray(cfg["w"][:k])
+    yo, wo = y0.copy(), w0.copy()
+    lo = orc.lyap(C3, prm, yo, wo, renorm_every=10, h=0.01, n_steps=1500, precision="f80")["lam"]
+    yg, wg = dev(y0), dev(w0)
+    lg = chs.lyap(C3, prm, yg, wg, renorm_every=10, h=0.01, n_steps=1500).cpu().numpy()
+    assert lam_err(lg, lo, 15.0) <= 1e-8
+    assert np.abs(wg.cpu().numpy() - wo).max() <= 1e-9 and rel_state(yg.cpu().numpy(), yo).max() <= 1e-10
+
+
+@pytest.mark.parametrize("k", [2, 3, 4, 5, 6])
+def test_coupled3_gali(chs, orc, k):
+    cfg = W.config("C4", n_ic=61)
+    y0, prm = cfg["y"], cfg["params"]
+    w0 = np.ascontiguousarray(cfg["w"][:k])
+    go = orc.gali(C3, prm, y0.copy(), w0.copy(), renorm_every=10, sample_every=30, h=0.01, n_steps=1500,
+                  precision="f80")["series"]
+    lg = dev(np.zeros((k, 61)))
+    gg = chs.gali(C3, prm, dev(y0), dev(w0), renorm_every=10, sample_every=30, lognorm=lg, h=0.01,
+                  n_steps=1500).cpu().numpy()
+    assert gg.shape == go.shape
+    assert go.min() > 1e-12 and np.abs(gg / go - 1).max() <= 1e-8
+    if k == 6:
+        # Liouville: the tangent map has determinant 1, so for 6 initially orthonormal vectors in the
+        # 6-dim phase space  GALI_6(t) * prod_v |w_v|(t) = |det| = 1, with prod |w_v| = exp(sum lognorm)
+        vol = gg[-1] * np.exp(lg.cpu().numpy().sum(0))
+        assert np.abs(vol - 1).max() <= 1e-10
+
+
+def test_coupled3_adaptive_mle_and_gali2(chs, orc):
+    cfg = W.config("C4", n_ic=50)
+    y0, prm = cfg["y"], cfg["params"]
+    st = dict(adaptive=True, t_end=30.0, rtol=1e-10, atol=1e-10)
+    w1 = np.ascontiguousarray(cfg["w"][:1])
+    lo = orc.lyap(C3, prm, y0.copy(), w1.copy(), renorm_every=1, precision="f80", **st)["lam"]
+    lg = chs.lyap(C3, prm, dev(y0), dev(w1), renorm_every=1, **st).cpu().numpy()
+    assert lam_err(lg, lo, 30.0) <= 1e-6
+    w2 = np.ascontiguousarray(cfg["w"][:2])
+    go = orc.gali(C3, prm, y0.copy(), w2.copy(), renorm_every=1, precision="f80", **st)["series"]
+    gg = chs.gali(C3, prm, dev(y0), dev(w2), renorm_every=1, **st).cpu().numpy()
+    assert np.abs(gg / go - 1).max() <= 1e-5
+    w6 = cfg["w"]
+    lo = orc.lyap(C3, prm, y0.copy(), w6.copy(), renorm_every=5, precision="f80", **st)["lam"]
+    lg = chs.lyap(C3, prm, dev(y0), dev(w6), renorm_every=5, **st).cpu().numpy()
+    assert lam_err(lg, lo, 30.0) <= 1e-6 and np.abs(lg.sum(0)).max() <= 1e-10
