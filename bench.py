@@ -30,12 +30,13 @@ sys.path.insert(0, ROOT)
 METRIC = "trajectory RK-steps/sec (FP64, incl. variational eqs)"
 UNIT = "RK-steps/s"
 # algorithmic FP64 flop per RK-step of the formulation that runs
-FLOP_PER_STEP = {"C2": 640.0, "C1sat": 1216.0, "C3": 1812.0, "C4": 4213.0, "C5": 8492.0}
+FLOP_PER_STEP = {"C2": 640.0, "C1sat": 1216.0, "C3": 1812.0, "C4": 4213.0, "C5": 8492.0, "F3": None}
 WORKLOAD_LABEL = {
-    "C1sat": "C1sat: Henon-Heiles fixed-step SALI kernel of configs[0] on a saturating 512x512 ensemble, 2000 steps",
+    "C1sat": "C1sat: Henon-Heiles fixed-step SALI kernel of configs[0] (h=0.01, renormalised every step) on a --sali-side^2 grid, --sali-steps steps",
     "C3": "C3: Henon-Heiles adaptive DOP8(5) rtol=atol=1e-12, 512x512 grid at E=1/6, t=1000, SALI (RK-step = attempted step)",
     "C4": "C4: 3-DoF coupled oscillators, 65536 ICs, full Lyapunov spectrum (6 vectors, MGS every 10 steps), h=0.01, 1e5 steps",
     "C5": "C5: FPUT-beta N=8, 65536 ICs, GALI_4 (renormalised every 10 steps), h=0.05, 2e4 steps",
+    "F3": "F3 (shape of PAPER.md Fig. 3): FPUT-beta chain, random ICs, GALI_4, adaptive DOP8(5) rtol=atol=1e-8, t=1000",
 }
 NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12  # 37.2
 
@@ -46,10 +47,14 @@ def parse():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C2", choices=["C2", "C1sat", "C3", "C4", "C5"])
+    ap.add_argument("--workload", default="C2", choices=["C2", "C1sat", "C3", "C4", "C5", "F3"])
     ap.add_argument("--shrink", type=int, default=1, help="C3/C4/C5: divide ensemble and horizon (profiling runs)")
     ap.add_argument("--side", type=int, default=1024, help="grid side per rank (C2)")
     ap.add_argument("--n-steps", type=int, default=5000, help="DOP8 steps per direction (C2)")
+    ap.add_argument("--sali-side", type=int, default=512, help="C1sat: grid side per rank")
+    ap.add_argument("--sali-steps", type=int, default=2000, help="C1sat: DOP8 steps")
+    ap.add_argument("--fput-n", type=int, default=8, help="F3: chain length (4, 8, 16, 32)")
+    ap.add_argument("--n-ic", type=int, default=1000, help="F3: ensemble size (PAPER.md:129: 10^3 random ICs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -104,10 +109,10 @@ def workload_inputs(args, rank, world):
         y0 = W.hh_grid(0.125, side * world, side, i_range=(rank * side, (rank + 1) * side))
         return dict(y0=y0, h=0.01, n_steps=args.n_steps, rk_steps=2.0 * y0.shape[1] * args.n_steps)
     # C1sat: the fixed-step SALI kernel of configs[0] on a saturating ensemble
-    side = 512
+    side = args.sali_side
     y0 = W.hh_grid(0.125, side * world, side, i_range=(rank * side, (rank + 1) * side))
     w0 = W.deviation_vectors(y0.shape[1], 2, 4, 0, "unit")
-    return dict(y0=y0, w0=w0, h=0.01, n_steps=2000, rk_steps=1.0 * y0.shape[1] * 2000)
+    return dict(y0=y0, w0=w0, h=0.01, n_steps=args.sali_steps, rk_steps=1.0 * y0.shape[1] * args.sali_steps)
 
 
 def oracle_sample(orc, args, target_s):
@@ -185,6 +190,24 @@ def make_workload(chs, torch, args, rank, world):
         call = lambda y, w: chs.sali(HH, None, y, w, renorm_every=1, h=wl["h"], n_steps=wl["n_steps"])
         host = lambda y, w, o: chs.sali_host(HH, None, y, w, o, renorm_every=1, h=wl["h"], n_steps=wl["n_steps"])
         out_rows, what, adaptive = 1, chs.WHAT_SALI, False
+    elif name == "F3":
+        # shape of the paper's Fig. 3: FPUT, 10^3 random ICs, GALI_4, adaptive
+        # solver, atol = 1e-8, tau = 10^3, as a function of the number of degrees of freedom
+        N = args.fput_n
+        sysid, prm = chs.SYS_FPUT, W.fput_params(N, 1.0, 0.0, 1.0)
+        y0_host = torch.from_numpy(W.fput_ics(args.n_ic, N, seed=2, E=0.125 * N)).pin_memory()
+        y0 = y0_host.cuda()
+        n_ic = y0.shape[1]
+        w0_np = W.deviation_vectors(n_ic, 4, 2 * N, 102, "orthonormal")
+        k = 4
+        rep = chs.Report(n_ic, "cuda")
+        t_end = 1000.0 / args.shrink
+        call = lambda y, w: chs.gali(sysid, prm, y, w, renorm_every=1, adaptive=True, t_end=t_end, rtol=1e-8,
+                                     atol=1e-8, report=rep)
+        host = lambda y, w, o: chs.gali_host(sysid, prm, y, w, o, renorm_every=1, adaptive=True, t_end=t_end,
+                                             rtol=1e-8, atol=1e-8)
+        out_rows, what, adaptive = 1, chs.WHAT_GALI, True
+        wl = dict(rk_steps=None, report=rep)
     else:
         n_full = {"C3": 512 * 512, "C4": 65536, "C5": 65536}[name]
         cfg = W.config(name, n_ic=max(1024, n_full // args.shrink) if args.shrink > 1 else None)
@@ -331,7 +354,7 @@ def main():
         return
 
     flop = FLOP_PER_STEP[args.workload]
-    achieved = flop * wl["rk_steps"] / (np.mean(ms) * 1e-3) / 1e12
+    achieved = (flop * wl["rk_steps"] / (np.mean(ms) * 1e-3) / 1e12) if flop else None
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * t_dev / args.steps, "higher_is_better": True,
@@ -341,14 +364,15 @@ def main():
                          "fixed DOP8 h=0.01, %d steps forward + %d backward" % (args.side, args.side, wl["n_steps"], wl["n_steps"]))
             if args.workload == "C2" else WORKLOAD_LABEL[args.workload] + (" (shrink %d)" % args.shrink if args.shrink > 1 else ""),
             "n_ic_per_gpu": int(n_ic), "rk_steps_per_step": wl["rk_steps"] * world,
+            "fput_n": args.fput_n if args.workload == "F3" else None,
             "l2": "flushed between timed iterations (256 MiB write)",
             "kernel": kinfo,
         },
         "roofline": {
             "bound": "alu", "achieved": achieved, "peak": NOMINAL_FP64_TFLOPS, "unit": "TFLOP/s",
-            "frac": achieved / NOMINAL_FP64_TFLOPS, "traffic": None,
+            "frac": (achieved / NOMINAL_FP64_TFLOPS) if achieved else None, "traffic": None,
             "peak_source": "nominal: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz (DESIGN.md Roofline)",
-            "measured_dfma_tflops": dfma_tflops, "frac_of_measured_dfma": achieved / dfma_tflops,
+            "measured_dfma_tflops": dfma_tflops, "frac_of_measured_dfma": (achieved / dfma_tflops) if achieved else None,
             "flop_per_rk_step": flop, "kernel_ms": float(np.mean(ms)),
         },
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
@@ -356,6 +380,8 @@ def main():
         "clocks": clocks,
         "wall_s_timed_region": t_wall,
     }
+    if "accepted" in wl:
+        out["config"]["accepted_steps"], out["config"]["rejected_steps"] = wl["accepted"], wl["rejected"]
     if not args.no_cpu_baseline and world == 1 and args.workload == "C2":
         from oracle import chaos_oracle as orc
         orc.build()
