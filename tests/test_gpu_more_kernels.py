@@ -166,3 +166,58 @@ def test_coupled3_adaptive_mle_and_gali2(chs, orc):
     lo = orc.lyap(C3, prm, y0.copy(), w6.copy(), renorm_every=5, precision="f80", **st)["lam"]
     lg = chs.lyap(C3, prm, dev(y0), dev(w6), renorm_every=5, **st).cpu().numpy()
     assert lam_err(lg, lo, 30.0) <= 1e-6 and np.abs(lg.sum(0)).max() <= 1e-10
+
+
+def _guarded(torch, shape, fill):
+    """A contiguous CUDA tensor of `shape` carved out of a larger allocation with canary words on
+    both sides (compute-sanitizer is closed on this pool: bounds are checked with guards instead)."""
+    n = int(np.prod(shape))
+    pad = 4096
+    buf = torch.full((n + 2 * pad,), 7.25e300, dtype=torch.float64, device="cuda")
+    view = buf[pad:pad + n].view(*shape)
+    view.copy_(torch.from_numpy(np.ascontiguousarray(fill)))
+    return buf, view, pad
+
+
+def _guards_intact(buf, pad):
+    return bool((buf[:pad] == 7.25e300).all().item() and (buf[-pad:] == 7.25e300).all().item())
+
+
+@pytest.mark.parametrize("case", ["hh_thread", "c3_tile", "fput_chain8", "fput_chain32"])
+def test_no_out_of_bounds_writes(chs, case):
+    import torch
+    n_ic = 37      # not a multiple of any tile or block size
+    if case == "hh_thread":
+        sysid, prm, y0 = HH, None, W.hh_grid(0.125, 37, 1)
+        w0 = W.deviation_vectors(n_ic, 2, 4, 1, "unit")
+    elif case == "c3_tile":
+        sysid, prm, y0 = C3, W.coupled3_params(0.1), W.coupled3_ics(n_ic, seed=1)
+        w0 = W.deviation_vectors(n_ic, 6, 6, 2, "orthonormal")
+    else:
+        N = 8 if case.endswith("8") else 32
+        sysid, prm, y0 = FPUT, W.fput_params(N, 1.0, 0.0, 1.0), W.fput_ics(n_ic, N, seed=2, E=0.125 * N)
+        w0 = W.deviation_vectors(n_ic, 4, 2 * N, 3, "orthonormal")
+    k = w0.shape[0]
+    by, y, pad = _guarded(torch, y0.shape, y0)
+    bw, w, _ = _guarded(torch, w0.shape, w0)
+    bl, lg, _ = _guarded(torch, (k, n_ic), np.zeros((k, n_ic)))
+    rep = chs.Report(n_ic, "cuda")
+    if case == "c3_tile":
+        lam = chs.lyap(sysid, prm, y, w, renorm_every=3, logsum=lg, report=rep, h=0.01, n_steps=50)
+        assert torch.isfinite(lam).all().item()
+        chs.lyap(sysid, prm, y, w, renorm_every=3, logsum=lg, adaptive=True, t_end=1.0, rtol=1e-9, atol=1e-9)
+    elif case == "hh_thread":
+        s = chs.sali(sysid, prm, y, w, renorm_every=1, sample_every=7, lognorm=lg, report=rep, h=0.01, n_steps=50)
+        assert s.shape == (50 // 7 + 1, n_ic) and torch.isfinite(s).all().item()
+        chs.sali(sysid, prm, y, w, renorm_every=1, lognorm=lg, adaptive=True, t_end=1.0, rtol=1e-9, atol=1e-9)
+    else:
+        g = chs.gali(sysid, prm, y, w, renorm_every=2, sample_every=5, lognorm=lg, report=rep, h=0.05, n_steps=40)
+        assert g.shape == (20 // 5 + 1, n_ic) and torch.isfinite(g).all().item()
+        chs.gali(sysid, prm, y, w, renorm_every=1, lognorm=lg, adaptive=True, t_end=2.0, rtol=1e-8, atol=1e-8)
+    bf, f, _ = _guarded(torch, (n_ic,), np.zeros(n_ic))
+    bb, b, _ = _guarded(torch, (n_ic,), np.zeros(n_ic))
+    chs.ld(sysid, prm, y, 0.0, 0.01, 20, out_fwd=f, out_bwd=b)
+    torch.cuda.synchronize()
+    for buf in (by, bw, bl, bf, bb):
+        assert _guards_intact(buf, pad)
+    assert torch.isfinite(y).all().item() and torch.isfinite(w).all().item() and (f > 0).all().item()
