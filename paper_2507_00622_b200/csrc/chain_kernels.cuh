@@ -105,22 +105,22 @@ struct Chain {
     __device__ __forceinline__ void renorm(bool want_log, bool apply) {
 #pragma unroll
         for (int v = 1; v < NCOL; v++) {
-            const double a = sqrt(dot(v, v));
-            const double inv = apply ? 1.0 / a : 1.0;
+            const double s = dot(v, v), ri = fast_rsqrt(s);
+            const double inv = apply ? ri : 1.0;
             q[v] *= inv;
             p[v] *= inv;
-            if (want_log && apply) lg[v] += log(a);
+            if (want_log && apply) lg[v] += log(s * ri);
         }
     }
     // modified Gram-Schmidt, right-looking order (see col_kernels.cuh)
     __device__ __forceinline__ void mgs(bool want_log, bool apply) {
 #pragma unroll
         for (int v = 1; v < NCOL; v++) {
-            const double r = sqrt(dot(v, v));
-            const double inv = apply ? 1.0 / r : 1.0;
+            const double s = dot(v, v), ri = fast_rsqrt(s);
+            const double inv = apply ? ri : 1.0;
             q[v] *= inv;
             p[v] *= inv;
-            if (want_log && apply) lg[v] += log(r);
+            if (want_log && apply) lg[v] += log(s * ri);
 #pragma unroll
             for (int u = v + 1; u < NCOL; u++) {
                 double dt = dot(v, u);

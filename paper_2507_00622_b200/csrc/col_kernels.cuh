@@ -202,14 +202,14 @@ struct Col {
 #pragma unroll
             for (int d = 0; d < ND; d++) s = fma(q[j * ND + d], q[j * ND + d], fma(p[j * ND + d], p[j * ND + d], s));
             const bool dev = is_dev(j) && apply;
-            const double a = sqrt(s);
-            const double inv = dev ? 1.0 / a : 1.0;
+            const double ri = fast_rsqrt(s);
+            const double inv = dev ? ri : 1.0;
 #pragma unroll
             for (int d = 0; d < ND; d++) {
                 q[j * ND + d] *= inv;
                 p[j * ND + d] *= inv;
             }
-            if (want_log && dev) lg[j] += log(a);
+            if (want_log && dev) lg[j] += log(s * ri);
         }
     }
 
@@ -232,7 +232,7 @@ struct Col {
             for (int d = 0; d < ND; d++) s = fma(wq[d], wq[d], s);
 #pragma unroll
             for (int d = 0; d < ND; d++) s = fma(wp[d], wp[d], s);
-            const double r = sqrt(s), inv = 1.0 / r;
+            const double inv = fast_rsqrt(s), r = s * inv;
 #pragma unroll
             for (int d = 0; d < ND; d++) {
                 wq[d] *= inv;
@@ -400,7 +400,7 @@ struct LdHook {
                 });
                 n2 = fma(P, P, fma(F[i][c], F[i][c], n2));
             }
-            M = fma(tab.bl[i], sqrt(tile_sum<C::L>(n2)), M);
+            M = fma(tab.bl[i], fast_sqrt(tile_sum<C::L>(n2)), M);
         }
     }
 };

@@ -23,7 +23,7 @@ struct HenonHeiles {
     struct Hess { double xx, xy, yy; };
     __device__ static __forceinline__ void force(const Params&, const double* Q, double* F) {
         const double x = Q[0], y = Q[1];
-        F[0] = -x - 2.0 * x * y;          // px' = -x - 2xy
+        F[0] = -x * fma(2.0, y, 1.0);     // px' = -x - 2xy = -x (1 + 2y)   (no 3-register DFMA)
         F[1] = fma(y, y, -y) - x * x;     // py' = -y - x^2 + y^2
     }
     // V_qq = [[1+2y, 2x],[2x, 1-2y]]
