@@ -372,9 +372,9 @@ def main():
             "bound": "alu", "achieved": achieved, "peak": NOMINAL_FP64_TFLOPS, "unit": "TFLOP/s",
             "frac": (achieved / NOMINAL_FP64_TFLOPS) if achieved else None,
             # DRAM bytes per launch from the ncu --set full capture of this kernel at this size
-            # (profiles/r01_ld_kernel_ncu.md: 33.66 MB read + 0.16 MB written; algorithmic 48 MiB, the
+            # (profiles/r01_ld_kernel_ncu.md: 33.70 MB read + 0.06 MB written; algorithmic 48 MiB, the
             # 16 MiB of results were still in L2 when the kernel ended); other workloads: not captured
-            "traffic": 33819648 if (args.workload == "C2" and args.side == 1024 and world == 1) else None,
+            "traffic": 33752832 if (args.workload == "C2" and args.side == 1024 and world == 1) else None,
             "peak_source": "nominal: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz (DESIGN.md Roofline)",
             "measured_dfma_tflops": dfma_tflops, "frac_of_measured_dfma": (achieved / dfma_tflops) if achieved else None,
             "flop_per_rk_step": flop, "kernel_ms": float(np.mean(ms)),
