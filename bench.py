@@ -48,7 +48,8 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C2", choices=["C2", "C1sat", "C3", "C4", "C5", "F3"])
-    ap.add_argument("--shrink", type=int, default=1, help="C3/C4/C5: divide ensemble and horizon (profiling runs)")
+    ap.add_argument("--shrink", type=int, default=1, help="C3/C4/C5/F3: divide the horizon (profiling runs)")
+    ap.add_argument("--shrink-ic", type=int, default=1, help="C3/C4/C5: divide the ensemble (profiling runs)")
     ap.add_argument("--side", type=int, default=1024, help="grid side per rank (C2)")
     ap.add_argument("--n-steps", type=int, default=5000, help="DOP8 steps per direction (C2)")
     ap.add_argument("--sali-side", type=int, default=512, help="C1sat: grid side per rank")
@@ -210,7 +211,7 @@ def make_workload(chs, torch, args, rank, world):
         wl = dict(rk_steps=None, report=rep)
     else:
         n_full = {"C3": 512 * 512, "C4": 65536, "C5": 65536}[name]
-        cfg = W.config(name, n_ic=max(1024, n_full // args.shrink) if args.shrink > 1 else None)
+        cfg = W.config(name, n_ic=max(1024, n_full // args.shrink_ic) if args.shrink_ic > 1 else None)
         sysid, prm, w0_np = cfg["system"], cfg["params"], cfg["w"]
         k = w0_np.shape[0]
         y0_host = torch.from_numpy(cfg["y"]).pin_memory()
