@@ -61,6 +61,7 @@ typedef double real;
 #define SYS_HENON_HEILES 0
 #define SYS_COUPLED3 1
 #define SYS_FPUT 2
+#define SYS_DOUBLE_PENDULUM 3 /* orbit only (no variational equations): PAPER.md:66-81 */
 
 /* per-trajectory status words */
 #define ST_OK 0
@@ -87,6 +88,7 @@ int orc_dim(int sys, const double *params)
         int N = (int)params[0];
         return N >= 1 ? 2 * N : -1;
     }
+    case SYS_DOUBLE_PENDULUM: return 4;
     }
     return -1;
 }
@@ -207,6 +209,58 @@ static real fput_energy(const double *P, const real *y)
     return H;
 }
 
+/* Dimensionless double pendulum, Eq.(1), Eq.(2), Eq.(3).
+ * y = (theta1, theta2, p1, p2); params = (sigma, alpha) (mass ratio, length ratio).  NOT
+ * separable: the kinetic energy depends on the angles.  Written exactly as printed:
+ *   theta' = B^-1(x) p,  x = cos(theta1 - theta2)
+ *   p'     = sin(Dtheta)/2 * (p^T C(x) p) * (1, -1)^T - (alpha (1+sigma) sin theta1, sin theta2)^T
+ *   C(x)   = -B^-1 (dB/dx) B^-1, formed here by the two matrix products,
+ * with B the inverse of Eq.(2): B = [[alpha^2 (1+sigma), alpha x],[alpha x, 1]], dB/dx = [[0,alpha],[alpha,0]].
+ * Orbit only: the paper prints no variational equations for this system. */
+static void dp_binv(real sg, real al, real x, real Bi[2][2])
+{
+    real den = 1 + sg - x * x;
+    Bi[0][0] = 1 / (al * al) / den;
+    Bi[0][1] = Bi[1][0] = -x / al / den;
+    Bi[1][1] = (1 + sg) / den;
+}
+static void dp_orbit(const double *P, const real *y, real *f)
+{
+    real sg = P[0], al = P[1];
+    real th1 = y[0], th2 = y[1], p1 = y[2], p2 = y[3];
+    real dth = th1 - th2;
+#ifdef ORC_REAL_IS_LONG_DOUBLE
+    real x = cosl(dth), sd = sinl(dth), s1 = sinl(th1), s2 = sinl(th2);
+#else
+    real x = cos(dth), sd = sin(dth), s1 = sin(th1), s2 = sin(th2);
+#endif
+    real Bi[2][2], dB[2][2] = {{0, al}, {al, 0}}, T[2][2], C[2][2];
+    dp_binv(sg, al, x, Bi);
+    for (int i = 0; i < 2; i++)
+        for (int j = 0; j < 2; j++) T[i][j] = Bi[i][0] * dB[0][j] + Bi[i][1] * dB[1][j];
+    for (int i = 0; i < 2; i++)
+        for (int j = 0; j < 2; j++) C[i][j] = -(T[i][0] * Bi[0][j] + T[i][1] * Bi[1][j]);
+    real pCp = p1 * (C[0][0] * p1 + C[0][1] * p2) + p2 * (C[1][0] * p1 + C[1][1] * p2);
+    f[0] = Bi[0][0] * p1 + Bi[0][1] * p2;
+    f[1] = Bi[1][0] * p1 + Bi[1][1] * p2;
+    f[2] = sd / 2 * pCp - al * (1 + sg) * s1;
+    f[3] = -(sd / 2 * pCp) - s2;
+}
+static real dp_energy(const double *P, const real *y)
+{
+    real sg = P[0], al = P[1];
+    real th1 = y[0], th2 = y[1], p1 = y[2], p2 = y[3];
+#ifdef ORC_REAL_IS_LONG_DOUBLE
+    real x = cosl(th1 - th2), c1 = cosl(th1), c2 = cosl(th2);
+#else
+    real x = cos(th1 - th2), c1 = cos(th1), c2 = cos(th2);
+#endif
+    real Bi[2][2];
+    dp_binv(sg, al, x, Bi);
+    real T = (p1 * (Bi[0][0] * p1 + Bi[0][1] * p2) + p2 * (Bi[1][0] * p1 + Bi[1][1] * p2)) / 2;
+    return T - al * (1 + sg) * c1 - c2;
+}
+
 /* f(y) for the augmented state  Y = (y, w_1, ..., w_k), each block of n components */
 static void rhs_aug(const prob_t *pb, const real *Y, real *F)
 {
@@ -224,6 +278,9 @@ static void rhs_aug(const prob_t *pb, const real *Y, real *F)
         fput_orbit(pb->params, Y, F);
         for (int v = 1; v <= pb->k; v++) fput_dev(pb->params, Y, Y + v * n, F + v * n);
         break;
+    case SYS_DOUBLE_PENDULUM:
+        dp_orbit(pb->params, Y, F); /* k = 0 only (checked by the entry points) */
+        break;
     }
 }
 
@@ -233,6 +290,7 @@ static real energy(const prob_t *pb, const real *y)
     case SYS_HENON_HEILES: return hh_energy(y);
     case SYS_COUPLED3: return c3_energy(pb->params, y);
     case SYS_FPUT: return fput_energy(pb->params, y);
+    case SYS_DOUBLE_PENDULUM: return dp_energy(pb->params, y);
     }
     return 0;
 }
@@ -616,6 +674,7 @@ int orc_run(int sys, const double *params, long long n_ic, double *y, double *w,
 {
     int n = orc_dim(sys, params);
     if (n < 0 || n_ic < 0 || k < 0 || (k > 0 && !w) || !y) return ORC_EINVAL;
+    if (sys == SYS_DOUBLE_PENDULUM && k > 0) return ORC_EINVAL; /* orbit only */
     if (mode != MODE_NONE && (k < 1 || renorm_every < 1)) return ORC_EINVAL;
     if (indicator == IND_SALI && k != 2) return ORC_EINVAL;
     if (indicator == IND_GALI && (k < 2 || k > n)) return ORC_EINVAL;

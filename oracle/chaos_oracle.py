@@ -19,7 +19,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "chaos_oracle.c")
 _LIBS = {}
 
-SYS_HENON_HEILES, SYS_COUPLED3, SYS_FPUT = 0, 1, 2
+SYS_HENON_HEILES, SYS_COUPLED3, SYS_FPUT, SYS_DOUBLE_PENDULUM = 0, 1, 2, 3
 MODE_NONE, MODE_NORM, MODE_MGS = 0, 1, 2
 IND_NONE, IND_SALI, IND_GALI = 0, 1, 2
 

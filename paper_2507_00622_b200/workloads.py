@@ -15,7 +15,7 @@ Layout of everything returned: float64, C-contiguous, component-major / IC-minor
 """
 import numpy as np
 
-SYS_HENON_HEILES, SYS_COUPLED3, SYS_FPUT = 0, 1, 2
+SYS_HENON_HEILES, SYS_COUPLED3, SYS_FPUT, SYS_DOUBLE_PENDULUM = 0, 1, 2, 3
 
 OMEGA_C3 = (1.0, 2.0 ** 0.5, 3.0 ** 0.5)
 
@@ -115,6 +115,17 @@ def fput_ics(n_ic, N=8, seed=2, E=1.0, k=1.0, beta=1.0, noise_var=1e-3):
     H4 = 0.25 * beta * (d ** 4).sum(1)
     s2 = (-H2 + np.sqrt(H2 * H2 + 4 * H4 * E)) / (2 * H4)
     return np.ascontiguousarray((z * np.sqrt(s2)[:, None]).T)
+
+
+# --------------------------------------------------------------------------- double pendulum
+def double_pendulum_ics(n_ic, seed=3, theta_max=2.0, p_max=1.0):
+    """Random ICs of the dimensionless double pendulum (the paper does not state its
+    IC set): angles uniform in [-theta_max, theta_max], momenta uniform in
+    [-p_max, p_max], order [ic][theta1, theta2, p1, p2] from default_rng(seed)."""
+    r = np.random.default_rng(seed).uniform(-1.0, 1.0, size=(n_ic, 4))
+    r[:, :2] *= theta_max
+    r[:, 2:] *= p_max
+    return np.ascontiguousarray(r.T)
 
 
 # --------------------------------------------------------------------------- the five configs
