@@ -30,12 +30,13 @@ sys.path.insert(0, ROOT)
 METRIC = "trajectory RK-steps/sec (FP64, incl. variational eqs)"
 UNIT = "RK-steps/s"
 # algorithmic FP64 flop per RK-step of the formulation that runs
-FLOP_PER_STEP = {"C2": 640.0, "C1sat": 1216.0, "C3": 1812.0, "C4": 4213.0, "C5": 8492.0, "F3": None}
+FLOP_PER_STEP = {"C2": 640.0, "C1sat": 1216.0, "C3": 1812.0, "C4": 4213.0, "C5": 8492.0, "F3": None, "F1": None}
 WORKLOAD_LABEL = {
     "C1sat": "C1sat: Henon-Heiles fixed-step SALI kernel of configs[0] (h=0.01, renormalised every step) on a --sali-side^2 grid, --sali-steps steps",
     "C3": "C3: Henon-Heiles adaptive DOP8(5) rtol=atol=1e-12, 512x512 grid at E=1/6, t=1000, SALI (RK-step = attempted step)",
     "C4": "C4: 3-DoF coupled oscillators, 65536 ICs, full Lyapunov spectrum (6 vectors, MGS every 10 steps), h=0.01, 1e5 steps",
     "C5": "C5: FPUT-beta N=8, 65536 ICs, GALI_4 (renormalised every 10 steps), h=0.05, 2e4 steps",
+    "F1": "F1 (shape of PAPER.md Fig. 1): dimensionless double pendulum (sigma = alpha = 1), random ICs, t = 1000, fixed h = 0.01 or adaptive rtol = atol = 1e-9",
     "F3": "F3 (shape of PAPER.md Fig. 3): FPUT-beta chain, random ICs, GALI_4, adaptive DOP8(5) rtol=atol=1e-8, t=1000",
 }
 NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12  # 37.2
@@ -47,7 +48,8 @@ def parse():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C2", choices=["C2", "C1sat", "C3", "C4", "C5", "F3"])
+    ap.add_argument("--workload", default="C2", choices=["C2", "C1sat", "C3", "C4", "C5", "F3", "F1"])
+    ap.add_argument("--f1-adaptive", action="store_true", help="F1: adaptive DOP8(5) instead of fixed step")
     ap.add_argument("--shrink", type=int, default=1, help="C3/C4/C5/F3: divide the horizon (profiling runs)")
     ap.add_argument("--shrink-ic", type=int, default=1, help="C3/C4/C5: divide the ensemble (profiling runs)")
     ap.add_argument("--side", type=int, default=1024, help="grid side per rank (C2)")
@@ -170,6 +172,32 @@ def make_workload(chs, torch, args, rank, world):
     from paper_2507_00622_b200 import workloads as W
     HH = chs.SYS_HENON_HEILES
     name = args.workload
+    if name == "F1":
+        # shape of the paper's Fig. 1: double pendulum, tau = 10^3, fixed vs adaptive
+        DPS, prm = chs.SYS_DOUBLE_PENDULUM, (1.0, 1.0)
+        y0_host = torch.from_numpy(W.double_pendulum_ics(args.n_ic, seed=3)).pin_memory()
+        y0 = y0_host.cuda()
+        n_ic = y0.shape[1]
+        yb, yh = torch.empty_like(y0), torch.empty_like(y0_host).pin_memory()
+        t_end = 1000.0 / args.shrink
+        if args.f1_adaptive:
+            rep = chs.Report(n_ic, "cuda")
+            call = lambda: chs.integrate_adaptive(DPS, prm, yb, 0.0, t_end, 1e-9, 1e-9, report=rep)
+            host = lambda: chs.integrate_host(DPS, prm, yh, adaptive=True, t_end=t_end, rtol=1e-9, atol=1e-9)
+            wl = dict(rk_steps=None, report=rep)
+        else:
+            ns = int(round(t_end / 0.01))
+            call = lambda: chs.integrate_fixed(DPS, prm, yb, 0.0, 0.01, ns)
+            host = lambda: chs.integrate_host(DPS, prm, yh, h=0.01, n_steps=ns)
+            wl = dict(rk_steps=1.0 * n_ic * ns)
+
+        def step_e2e():
+            yh.copy_(y0_host)
+            host()
+
+        return dict(wl=wl, n_ic=n_ic, h2d=y0_host.numel() * 8, d2h=y0_host.numel() * 8,
+                    kinfo=chs.kernel_info(DPS, prm, chs.WHAT_INTEGRATE, adaptive=args.f1_adaptive, n_ic=n_ic),
+                    step_dev=call, step_e2e=step_e2e, prepare=lambda: yb.copy_(y0))
     if name in ("C2", "C1sat"):
         wl = workload_inputs(args, rank, world)
         y0_host = torch.from_numpy(wl["y0"]).pin_memory()

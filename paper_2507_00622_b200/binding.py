@@ -16,7 +16,7 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libchaoticus.so")
 
-SYS_HENON_HEILES, SYS_COUPLED3, SYS_FPUT = 0, 1, 2
+SYS_HENON_HEILES, SYS_COUPLED3, SYS_FPUT, SYS_DOUBLE_PENDULUM = 0, 1, 2, 3
 WHAT_INTEGRATE, WHAT_SALI, WHAT_GALI, WHAT_LD, WHAT_LYAP = 0, 1, 2, 3, 4
 ST_OK, ST_NONFINITE, ST_UNDERFLOW, ST_MAXSTEPS = 0, 1, 2, 3
 

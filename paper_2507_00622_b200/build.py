@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 BUILD = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libchaoticus.so")
 UNITS = ["chaoticus", "probe", "inst_hh", "inst_hh_ind", "inst_hh_adapt", "inst_c3", "inst_c3_lyap", "inst_fput",
-         "inst_fput_adapt", "inst_fput_n4", "inst_fput_n16", "inst_fput_n32", "inst_hh_adapt2", "inst_c3_more"]
+         "inst_fput_adapt", "inst_fput_n4", "inst_fput_n16", "inst_fput_n32", "inst_hh_adapt2", "inst_c3_more", "inst_dp"]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xptxas", "-v",
               "-Xcompiler", "-fPIC"]
 

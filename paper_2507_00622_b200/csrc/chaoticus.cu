@@ -51,6 +51,8 @@ int dim_of(const chs_problem* pb, int* fput_n) {
     switch (pb->system) {
         case CHS_SYS_HENON_HEILES: return 4;
         case CHS_SYS_COUPLED3: return (pb->params && pb->n_params >= 4) ? 6 : -1;
+        case CHS_SYS_DOUBLE_PENDULUM:
+            return (pb->params && pb->n_params >= 2 && pb->params[1] > 0.0 && pb->params[0] > -1.0) ? 4 : -1;
         case CHS_SYS_FPUT: {
             if (!pb->params || pb->n_params < 4) return -1;
             const double Nd = pb->params[0];
@@ -76,6 +78,7 @@ int dispatch(const chs::LaunchReq& rq) {
     if ((r = chs::try_launch_fput_n32(rq)) != -1) return r;
     if ((r = chs::try_launch_hh_adapt2(rq)) != -1) return r;
     if ((r = chs::try_launch_c3_more(rq)) != -1) return r;
+    if ((r = chs::try_launch_dp(rq)) != -1) return r;
     return -1;
 }
 

@@ -38,6 +38,7 @@ int try_launch_fput_n16(const LaunchReq& rq);
 int try_launch_fput_n32(const LaunchReq& rq);
 int try_launch_hh_adapt2(const LaunchReq& rq);
 int try_launch_c3_more(const LaunchReq& rq);
+int try_launch_dp(const LaunchReq& rq);
 
 template <class Kern>
 inline int finish_launch(const LaunchReq& rq, Kern kern, int tpb, int lanes, long long n_threads) {

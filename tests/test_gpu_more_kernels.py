@@ -221,3 +221,58 @@ def test_no_out_of_bounds_writes(chs, case):
     for buf in (by, bw, bl, bf, bb):
         assert _guards_intact(buf, pad)
     assert torch.isfinite(y).all().item() and torch.isfinite(w).all().item() and (f > 0).all().item()
+
+
+# ---------------------------------------------------------------------------- double pendulum (generic kernel)
+DP = W.SYS_DOUBLE_PENDULUM
+
+
+@pytest.mark.parametrize("prm", [(1.0, 1.0), (0.5, 2.0)])
+def test_double_pendulum_fixed(chs, orc, prm):
+    """non-separable system through the generic first-order kernel."""
+    y0 = W.double_pendulum_ics(333, seed=3)
+    yo = y0.copy()
+    orc.integrate_fixed(DP, prm, yo, 0.0, 0.01, 1000, precision="f80")
+    yg = dev(y0)
+    rep = chs.Report(333, "cuda")
+    chs.integrate_fixed(DP, prm, yg, 0.0, 0.01, 1000, report=rep)
+    assert (rep.status.cpu().numpy() == 0).all()
+    # t = 10 is well inside 10 Lyapunov times for these energies
+    assert rel_state(yg.cpu().numpy(), yo).max() <= 1e-10
+    # energy conservation on the GPU result (paper's level for Fig. 1: 1e-9, PAPER.md:121)
+    # (truncation error of the method itself at h = 0.01: the oracle drifts by the same amount)
+    H0, H1 = orc.energy(DP, prm, y0), orc.energy(DP, prm, yg.cpu().numpy())
+    Ho = orc.energy(DP, prm, yo)
+    assert np.abs(H1 - H0).max() <= 1e-10 and np.abs(H1 - Ho).max() <= 1e-12
+    # backward
+    yo = y0.copy()
+    orc.integrate_fixed(DP, prm, yo, 0.0, -0.01, 500, precision="f80")
+    yg = dev(y0)
+    chs.integrate_fixed(DP, prm, yg, 0.0, -0.01, 500)
+    assert rel_state(yg.cpu().numpy(), yo).max() <= 1e-10
+
+
+def test_double_pendulum_adaptive(chs, orc):
+    prm = (1.0, 1.0)
+    y0 = W.double_pendulum_ics(200, seed=4)
+    yo = y0.copy()
+    ro = orc.integrate_adaptive(DP, prm, yo, 0.0, 15.0, 1e-11, 1e-11, precision="f80")
+    yg = dev(y0)
+    rep = chs.Report(200, "cuda")
+    chs.integrate_adaptive(DP, prm, yg, 0.0, 15.0, 1e-11, 1e-11, report=rep)
+    assert (rep.status.cpu().numpy() == 0).all() and (rep.t_final.cpu().numpy() == 15.0).all()
+    lam_guard = rel_state(yg.cpu().numpy(), yo)
+    assert np.median(lam_guard) <= 1e-9 and lam_guard.max() <= 1e-6     # chaotic orbits amplify the tolerance
+    assert abs(rep.n_accepted.cpu().numpy().sum() / ro["n_accepted"].sum() - 1) <= 5e-3
+    H0, H1 = orc.energy(DP, prm, y0), orc.energy(DP, prm, yg.cpu().numpy())
+    assert np.abs(H1 - H0).max() <= 1e-9
+
+
+def test_double_pendulum_unsupported_entry_points(chs):
+    import torch
+    y = dev(W.double_pendulum_ics(8))
+    w = torch.zeros((2, 4, 8), dtype=torch.float64, device="cuda")
+    with pytest.raises(chs.ChaoticusError, match="no compiled kernel"):
+        chs.sali(DP, (1.0, 1.0), y, w, h=0.01, n_steps=10)
+    with pytest.raises(chs.ChaoticusError):
+        chs.integrate_fixed(DP, (1.0, -1.0), y, 0.0, 0.01, 10)    # alpha <= 0
