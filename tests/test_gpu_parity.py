@@ -208,6 +208,23 @@ def test_sali_fixed_hh(chs, orc):
     assert np.abs(nrm - 1).max() <= 1e-14
 
 
+def test_sali_fixed_hh_thread_layout(chs, orc):
+    """Above 4096 trajectories chaoticus_sali switches from the 4-lane tile to one thread per
+    trajectory (the kernel bench.py --workload C1sat times): same parity bar."""
+    y0, w0 = _sali_case(67)          # 4489 ICs
+    n_ic = y0.shape[1]
+    assert chs.kernel_info(HH, None, chs.WHAT_SALI, k=2, n_ic=n_ic)["lanes"] == 1
+    assert chs.kernel_info(HH, None, chs.WHAT_SALI, k=2, n_ic=1024)["lanes"] == 4
+    yo, wo, lo = y0.copy(), w0.copy(), np.zeros((2, n_ic))
+    so = orc.sali(HH, None, yo, wo, renorm_every=1, sample_every=200, lognorm=lo, h=0.01, n_steps=600,
+                  precision="f80")["series"]
+    yg, wg, lg = dev(y0), dev(w0), dev(np.zeros((2, n_ic)))
+    sg = chs.sali(HH, None, yg, wg, renorm_every=1, sample_every=200, lognorm=lg, h=0.01, n_steps=600).cpu().numpy()
+    assert rel_state(yg.cpu().numpy(), yo).max() <= TOL_STATE
+    assert np.abs(sg / so - 1).max() <= TOL_IND
+    assert np.abs(wg.cpu().numpy() - wo).max() <= 1e-9 and np.abs(lg.cpu().numpy() - lo).max() <= 1e-9
+
+
 def test_sali_renorm_interval_and_tail(chs, orc):
     """m = 7 does not divide n_steps = 1000: a final renormalisation happens at the end."""
     y0, w0 = _sali_case(10)
