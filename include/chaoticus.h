@@ -50,8 +50,8 @@ typedef enum { CHS_OK = 0, CHS_EINVAL = 1, CHS_EUNSUPPORTED = 2, CHS_ECUDA = 3 }
  *  CHS_SYS_DOUBLE_PENDULUM  n = 4, params (sigma, alpha) = (mass ratio, length ratio); state
  *                        (theta1, theta2, p1, p2).  NOT separable: Eq.(1)
  *                        Eq.(2), Eq.(3).  Orbit only: chaoticus_integrate_fixed /
- *                        _adaptive (generic first-order kernel); every other entry point returns
- *                        CHS_EUNSUPPORTED for it. */
+ *                        _adaptive and chaoticus_ld (generic first-order kernel); the entry points
+ *                        that need variational equations return CHS_EUNSUPPORTED for it. */
 typedef enum { CHS_SYS_HENON_HEILES = 0, CHS_SYS_COUPLED3 = 1, CHS_SYS_FPUT = 2, CHS_SYS_DOUBLE_PENDULUM = 3 } chs_system;
 
 typedef struct {

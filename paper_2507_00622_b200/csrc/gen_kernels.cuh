@@ -233,4 +233,51 @@ gen_run_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, 
 }
 
 #undef CHS_GEN_ADVANCE
+
+// Lagrangian descriptor with the generic form: M += |h| sum_i b_i |K_i|_2,
+// K_i the full stage derivative.  One thread per (direction, IC); the backward pass is the forward
+// pass of (theta, -p): the kinetic energy is a quadratic form in p, so H is even in p.
+template <class Sys, int TPB, int MINB>
+__global__ void __launch_bounds__(TPB, MINB)
+gen_ld_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, const RunArgs a, int dir_first,
+              int n_dirs) {
+    constexpr int N = Sys::N;
+    const long long gt = (long long)blockIdx.x * TPB + threadIdx.x;
+    if (gt >= a.n_ic * n_dirs) return;
+    const int dsel = dir_first + (int)(gt / a.n_ic);
+    const long long ic = gt % a.n_ic;
+    const double psign = dsel == 0 ? 1.0 : -1.0;
+    double y[N];
+#pragma unroll
+    for (int c = 0; c < N; c++) y[c] = a.y0[(long long)c * a.n_ic + ic] * (c >= N / 2 ? psign : 1.0);
+    double M = 0.0;
+    for (long long st = 0; st < a.n_steps; ++st) {
+        double K[12][N];
+        dop8_generic_stages<Sys, true>(tab, prm, 0.0, y, K);
+        static_for<0, 12>([&](auto lc) {
+            constexpr int l = decltype(lc)::value;
+            if constexpr (coef::B[l] != 0.0) {
+                double n2 = 0.0;
+#pragma unroll
+                for (int c = 0; c < N; c++) n2 = fma(K[l][c], K[l][c], n2);
+                M = fma(tab.bl[l], fast_sqrt(n2), M);
+            }
+        });
+#pragma unroll
+        for (int c = 0; c < N; c++) {
+            double s = y[c];
+            static_for<0, 12>([&](auto lc) {
+                constexpr int l = decltype(lc)::value;
+                if constexpr (coef::B[l] != 0.0) s = fma(tab.bp[l], K[l][c], s);
+            });
+            y[c] = s;
+        }
+    }
+    bool ok = true;
+#pragma unroll
+    for (int c = 0; c < N; c++) ok = ok && isfinite(y[c]);
+    double* out = dsel == 0 ? a.ld_fwd : a.ld_bwd;
+    out[ic] = ok ? M : nan("");
+}
+
 }  // namespace chs

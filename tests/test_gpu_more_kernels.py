@@ -276,3 +276,13 @@ def test_double_pendulum_unsupported_entry_points(chs):
         chs.sali(DP, (1.0, 1.0), y, w, h=0.01, n_steps=10)
     with pytest.raises(chs.ChaoticusError):
         chs.integrate_fixed(DP, (1.0, -1.0), y, 0.0, 0.01, 10)    # alpha <= 0
+
+
+def test_double_pendulum_ld(chs, orc):
+    """LD of the non-separable system (no variational equations needed)."""
+    prm = (0.5, 2.0)
+    y0 = W.double_pendulum_ics(301, seed=6)
+    fo, bo = orc.ld(DP, prm, y0, 0.0, 0.01, 800, precision="f80")
+    f, b = chs.ld(DP, prm, dev(y0), 0.0, 0.01, 800)
+    assert np.abs(f.cpu().numpy() / fo - 1).max() <= 1e-8 and np.abs(b.cpu().numpy() / bo - 1).max() <= 1e-8
+    assert (fo > 0).all() and np.abs(fo - bo).max() > 1e-3        # the two directions really differ
