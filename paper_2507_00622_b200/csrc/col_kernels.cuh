@@ -513,7 +513,7 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
             bool ren = false;
             if (active) {
                 if (err < 1.0) {
-                    double factor = (err == 0.0) ? 10.0 : fmin(10.0, 0.9 / root8(err));
+                    double factor = (err == 0.0) ? 10.0 : fmin(10.0, 0.9 * inv_root8(err));
                     if (rejected) factor = fmin(factor, 1.0);
                     h_abs = h_try * factor;
                     t = t_new;
@@ -535,7 +535,7 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
                         ren = true;
                     }
                 } else if (err >= 1.0) {
-                    h_abs = h_try * fmax(0.2, 0.9 / root8(err));
+                    h_abs = h_try * fmax(0.2, 0.9 * inv_root8(err));
                     rejected = true;
                     n_rej++;
                 } else {
@@ -545,8 +545,8 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
             if constexpr (MODE != MODE_NONE) {
                 if (__any_sync(0xffffffffu, ren)) s.template do_renorm<MODE>(want_log, ren);
             }
-            const bool fin = s.finite_all();  // tile-wide, warp-convergent
-            if (active && !fin) status = ST_NONFINITE;
+            // a non-finite y+ needs no separate test here: inf or NaN in y+ makes its error scale, hence
+            // err, NaN (fast_rcp(inf) is NaN), which the branch above turns into ST_NONFINITE
         }
     }
     // ---- outputs ------------------------------------------------------------------------------

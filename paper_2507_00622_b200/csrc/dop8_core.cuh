@@ -67,6 +67,43 @@ __device__ __forceinline__ bool tile_any(bool b) {
     }
 }
 
+// ---- square roots off the slow path ----------------------------------------------------------
+// MUFU.RSQ64H seed y0 (|1 - x y0^2| <= 2^-19, measured) and the cubic Taylor polynomial of
+// (1-e)^(-1/2): relative error <= 1 ulp (measured against sqrt() over 1.6e8 arguments), 6 FP64
+// instructions none of which reads three distinct registers (DESIGN.md "Roofline": those run at
+// 2/3 rate), no branch.  The library sqrt()/1.0/sqrt() cost 8 + ~10 instructions and a slow-path
+// branch.  Arguments are sums of squares: x >= 0.
+__device__ __forceinline__ double rsqrt_seed(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    return y;
+}
+// 1/sqrt(x); x = 0 (or denormal) gives inf, as 1.0/sqrt(0.0) does
+__device__ __forceinline__ double fast_rsqrt(double x) {
+    const double y0 = rsqrt_seed(x);
+    const double e = fma(-(x * y0), y0, 1.0);
+    const double t = fma(e, fma(e, 0.3125, 0.375), 0.5);
+    return fma(y0, e * t, y0);
+}
+// sqrt(x); x = 0 (or denormal) gives 0
+__device__ __forceinline__ double fast_sqrt(double x) {
+    const double y0 = rsqrt_seed(x);
+    const double g0 = x * y0;
+    const double e = fma(-g0, y0, 1.0);
+    const double t = fma(e, fma(e, 0.3125, 0.375), 0.5);
+    const double r = fma(g0, e * t, g0);
+    return (__double2hiint(x) < 0x00100000) ? 0.0 : r;  // integer test: stays off the FP64 pipe
+}
+
+// 1/x for x > 0 (error-norm scales): MUFU.RCP64H seed r0, e = 1 - x r0, r = r0 (1 + e + e^2 + e^3...)
+// truncated after e^3 (|e| <= 2^-19: error 2^-76): 3 FP64 instructions, no slow-path branch.
+__device__ __forceinline__ double fast_rcp(double x) {
+    double r0;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r0) : "d"(x));
+    const double e = fma(-x, r0, 1.0);
+    return fma(r0, fma(e, fma(e, e, e), e), r0);
+}
+
 // ---- stages -------------------------------------------------------------------------------
 // force(Q, Fout): evaluates the NI force components at the stage coordinates Q.
 // hook(Int<i>, F): called after stage i's force is available (used by the LD quadrature).
@@ -178,8 +215,8 @@ __device__ __forceinline__ void dop8_error_sums(const Tab& tab, double h, const 
             if constexpr (coef::E5[l] != 0.0) s5p = fma(tab.e5p[l], F[l][c], s5p);
             if constexpr (coef::E3[l] != 0.0) s3p = fma(tab.e3p[l], F[l][c], s3p);
         });
-        double iq = 1.0 / fma(rtol, fmax(fabs(q[c]), fabs(qn[c])), atol);
-        double ip = 1.0 / fma(rtol, fmax(fabs(p[c]), fabs(pn[c])), atol);
+        double iq = fast_rcp(fma(rtol, fmax(fabs(q[c]), fabs(qn[c])), atol));
+        double ip = fast_rcp(fma(rtol, fmax(fabs(p[c]), fabs(pn[c])), atol));
         double a = h * s5q * iq, b = s5p * ip, c3 = h * s3q * iq, d3 = s3p * ip;
         if (on[c]) {
             S5 = fma(a, a, fma(b, b, S5));
@@ -188,38 +225,12 @@ __device__ __forceinline__ void dop8_error_sums(const Tab& tab, double h, const 
     }
 }
 
-// ---- square roots off the slow path ----------------------------------------------------------
-// MUFU.RSQ64H seed y0 (|1 - x y0^2| <= 2^-19, measured) and the cubic Taylor polynomial of
-// (1-e)^(-1/2): relative error <= 1 ulp (measured against sqrt() over 1.6e8 arguments), 6 FP64
-// instructions none of which reads three distinct registers (DESIGN.md "Roofline": those run at
-// 2/3 rate), no branch.  The library sqrt()/1.0/sqrt() cost 8 + ~10 instructions and a slow-path
-// branch.  Arguments are sums of squares: x >= 0.
-__device__ __forceinline__ double rsqrt_seed(double x) {
-    double y;
-    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    return y;
-}
-// 1/sqrt(x); x = 0 (or denormal) gives inf, as 1.0/sqrt(0.0) does
-__device__ __forceinline__ double fast_rsqrt(double x) {
-    const double y0 = rsqrt_seed(x);
-    const double e = fma(-(x * y0), y0, 1.0);
-    const double t = fma(e, fma(e, 0.3125, 0.375), 0.5);
-    return fma(y0, e * t, y0);
-}
-// sqrt(x); x = 0 (or denormal) gives 0
-__device__ __forceinline__ double fast_sqrt(double x) {
-    const double y0 = rsqrt_seed(x);
-    const double g0 = x * y0;
-    const double e = fma(-g0, y0, 1.0);
-    const double t = fma(e, fma(e, 0.3125, 0.375), 0.5);
-    const double r = fma(g0, e * t, g0);
-    return (__double2hiint(x) < 0x00100000) ? 0.0 : r;  // integer test: stays off the FP64 pipe
-}
-
 // per-trajectory status words (include/chaoticus.h CHS_ST_*)
 enum : int { ST_OK = 0, ST_NONFINITE = 1, ST_UNDERFLOW = 2, ST_MAXSTEPS = 3 };
 
 // x^(1/8) by three square roots (the controller's exponent)
 __device__ __forceinline__ double root8(double x) { return sqrt(sqrt(sqrt(x))); }
+// x^(-1/8), x > 0 finite: branch-free (used once per attempt by the step-size controller)
+__device__ __forceinline__ double inv_root8(double x) { return fast_rsqrt(fast_sqrt(fast_sqrt(x))); }
 
 }  // namespace chs

@@ -190,14 +190,14 @@ gen_run_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, 
             CHS_GEN_ADVANCE()
 #pragma unroll
             for (int c = 0; c < N; c++) {
-                const double is = 1.0 / fma(a.rtol, fmax(fabs(y[c]), fabs(yn[c])), a.atol);
+                const double is = fast_rcp(fma(a.rtol, fmax(fabs(y[c]), fabs(yn[c])), a.atol));
                 const double u = K[0][c] * is, v = K[1][c] * is;
                 S5 = fma(u, u, S5);
                 S3 = fma(v, v, S3);
             }
             const double err = (S5 == 0.0 && S3 == 0.0) ? 0.0 : h_try * S5 / sqrt((S5 + 0.01 * S3) * (double)N);
             if (err < 1.0) {
-                double factor = (err == 0.0) ? 10.0 : fmin(10.0, 0.9 / root8(err));
+                double factor = (err == 0.0) ? 10.0 : fmin(10.0, 0.9 * inv_root8(err));
                 if (rejected) factor = fmin(factor, 1.0);
                 h_abs = h_try * factor;
                 t = t_new;
@@ -212,7 +212,7 @@ gen_run_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, 
                 rejected = false;
                 if (!fin) status = ST_NONFINITE;
             } else if (err >= 1.0) {
-                h_abs = h_try * fmax(0.2, 0.9 / root8(err));
+                h_abs = h_try * fmax(0.2, 0.9 * inv_root8(err));
                 rejected = true;
                 n_rej++;
             } else {

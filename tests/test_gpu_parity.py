@@ -470,3 +470,19 @@ def test_gali_adaptive_fput(chs, orc):
     assert (rep.status.cpu().numpy() == 0).all()
     assert np.abs(gg / ro["series"] - 1).max() <= 1e-4          # both solve to tolerance 1e-8
     assert abs(rep.n_accepted.cpu().numpy().sum() / ro["n_accepted"].sum() - 1) <= 1e-2
+
+
+def test_adaptive_escaping_orbit_status(chs):
+    """An escaping Henon-Heiles orbit blows up in finite time: the adaptive solver must flag it
+    (non-finite state or step-size underflow), return NaN for it, and leave its neighbours alone."""
+    y0 = W.hh_grid(0.125, 5, 5)
+    y0[:, 7] = [0.0, 3.0, 0.0, 5.0]
+    yg = dev(y0)
+    rep = chs.Report(25, "cuda")
+    chs.integrate_adaptive(HH, None, yg, 0.0, 200.0, 1e-10, 1e-10, max_steps=200000, report=rep)
+    st = rep.status.cpu().numpy()
+    out = yg.cpu().numpy()
+    assert st[7] in (chs.ST_NONFINITE, chs.ST_UNDERFLOW) and np.isnan(out[:, 7]).all()
+    ok = np.delete(np.arange(25), 7)
+    assert (st[ok] == 0).all() and np.isfinite(out[:, ok]).all()
+    assert (rep.t_final.cpu().numpy()[ok] == 200.0).all()
