@@ -27,13 +27,13 @@ struct Chain {
     Params prm;
     int lt;
     double q[NI], p[NI];
-    double lg[NCOL];  // lg[v], v >= 1: identical on all lanes of the tile
+    LogAcc lg[NCOL];  // deferred-log accumulators, lg[v], v >= 1: identical on all lanes of the tile
 
     __device__ __forceinline__ void init(const Params& P) {
         prm = P;
         lt = (int)(threadIdx.x % L);
 #pragma unroll
-        for (int j = 0; j < NCOL; j++) lg[j] = 0.0;
+        for (int j = 0; j < NCOL; j++) logacc_init(lg[j]);
     }
     __device__ __forceinline__ void load(const double* y, const double* w, long long n_ic, long long ic,
                                          double psign) {
@@ -59,8 +59,9 @@ struct Chain {
 #pragma unroll
         for (int v = 1; v < NCOL; v++) {
             const long long o = (long long)(v - 1) * a.n_ic + ic;
-            if (a.logacc) a.logacc[o] = bad ? nan("") : a.logacc[o] + lg[v];
-            if (a.lambda) a.lambda[o] = (bad || elapsed == 0.0) ? nan("") : lg[v] / elapsed;
+            const double lv = logacc_value(lg[v]);
+            if (a.logacc) a.logacc[o] = bad ? nan("") : a.logacc[o] + lv;
+            if (a.lambda) a.lambda[o] = (bad || elapsed == 0.0) ? nan("") : lv / elapsed;
         }
     }
     __device__ __forceinline__ void on_mask(bool (&on)[NI]) const {
@@ -109,7 +110,7 @@ struct Chain {
             const double inv = apply ? ri : 1.0;
             q[v] *= inv;
             p[v] *= inv;
-            if (want_log && apply) lg[v] += log(s * ri);
+            if (want_log && apply) logacc_mul(lg[v], s * ri);
         }
     }
     // modified Gram-Schmidt, right-looking order (see col_kernels.cuh)
@@ -120,7 +121,7 @@ struct Chain {
             const double inv = apply ? ri : 1.0;
             q[v] *= inv;
             p[v] *= inv;
-            if (want_log && apply) lg[v] += log(s * ri);
+            if (want_log && apply) logacc_mul(lg[v], s * ri);
 #pragma unroll
             for (int u = v + 1; u < NCOL; u++) {
                 double dt = dot(v, u);

@@ -108,7 +108,7 @@ struct Col {
     int lt;          // lane in tile
     double s_lane;   // 1/2 on the orbit lane of a multi-lane tile, else 1
     double q[NI], p[NI];
-    double lg[CPL];  // log accumulators of this lane's columns
+    LogAcc lg[CPL];  // deferred-log accumulators of this lane's columns
 
     __device__ __forceinline__ int col_of(int j) const { return lt * CPL + j; }
     __device__ __forceinline__ bool is_dev(int j) const {
@@ -121,7 +121,7 @@ struct Col {
         lt = (L == 1) ? 0 : (int)(threadIdx.x % L);
         s_lane = (L > 1 && lt == 0) ? 0.5 : 1.0;
 #pragma unroll
-        for (int j = 0; j < CPL; j++) lg[j] = 0.0;
+        for (int j = 0; j < CPL; j++) logacc_init(lg[j]);
     }
 
     __device__ __forceinline__ void load(const double* y, const double* w, long long n_ic, long long ic,
@@ -209,7 +209,7 @@ struct Col {
                 q[j * ND + d] *= inv;
                 p[j * ND + d] *= inv;
             }
-            if (want_log && dev) lg[j] += log(s * ri);
+            if (want_log && dev) logacc_mul(lg[j], s * ri);
         }
     }
 
@@ -245,7 +245,7 @@ struct Col {
                     q[jv * ND + d] = wq[d];
                     p[jv * ND + d] = wp[d];
                 }
-                if (want_log) lg[jv] += log(r);
+                if (want_log) logacc_mul(lg[jv], r);
             }
 #pragma unroll
             for (int j = 0; j < CPL; j++) {
@@ -321,8 +321,9 @@ struct Col {
             for (int j = 0; j < CPL; j++) {
                 if (is_dev(j)) {
                     const long long o = (long long)(col_of(j) - 1) * a.n_ic + ic;
-                    if (a.logacc) a.logacc[o] = bad ? nan("") : a.logacc[o] + lg[j];
-                    if (a.lambda) a.lambda[o] = (bad || elapsed == 0.0) ? nan("") : lg[j] / elapsed;
+                    const double lv = logacc_value(lg[j]);
+                    if (a.logacc) a.logacc[o] = bad ? nan("") : a.logacc[o] + lv;
+                    if (a.lambda) a.lambda[o] = (bad || elapsed == 0.0) ? nan("") : lv / elapsed;
                 }
             }
         }
@@ -508,7 +509,7 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
             dop8_error_sums<NI>(tab, h, s.q, s.p, qn, pn, F, a.rtol, a.atol, on, S5, S3);
             S5 = tile_sum<L>(S5);
             S3 = tile_sum<L>(S3);
-            const double err = (S5 == 0.0 && S3 == 0.0) ? 0.0 : h_try * S5 / sqrt((S5 + 0.01 * S3) * (double)C::D);
+            const double err = (S5 == 0.0 && S3 == 0.0) ? 0.0 : h_try * S5 * fast_rsqrt((S5 + 0.01 * S3) * (double)C::D);
 
             bool ren = false;
             if (active) {

@@ -104,6 +104,29 @@ __device__ __forceinline__ double fast_rcp(double x) {
     return fma(r0, fma(e, fma(e, e, e), e), r0);
 }
 
+// ---- deferred logarithm ----------------------------------------------------------------------
+// sum_k ln(r_k) of the renormalisation factors is kept as a running PRODUCT in
+// (mantissa in [1,2), integer exponent) form: one DMUL and a few integer instructions per factor
+// instead of a ~45-instruction log() with a slow-path branch; the logarithm is taken once, when the
+// accumulator is written out.  (Also more accurate than summing rounded logarithms.)
+struct LogAcc {
+    double m;
+    int e;
+};
+__device__ __forceinline__ void logacc_init(LogAcc& a) {
+    a.m = 1.0;
+    a.e = 0;
+}
+__device__ __forceinline__ void logacc_mul(LogAcc& a, double r) {  // r > 0, finite, normal
+    const double t = a.m * r;
+    const int hi = __double2hiint(t);
+    a.e += ((hi >> 20) & 0x7ff) - 1023;
+    a.m = __hiloint2double((hi & 0x800fffff) | 0x3ff00000, __double2loint(t));
+}
+__device__ __forceinline__ double logacc_value(const LogAcc& a) {
+    return fma((double)a.e, 0.693147180559945309417232, log(a.m));
+}
+
 // ---- stages -------------------------------------------------------------------------------
 // force(Q, Fout): evaluates the NI force components at the stage coordinates Q.
 // hook(Int<i>, F): called after stage i's force is available (used by the LD quadrature).

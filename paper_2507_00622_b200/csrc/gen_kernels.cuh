@@ -195,7 +195,7 @@ gen_run_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, 
                 S5 = fma(u, u, S5);
                 S3 = fma(v, v, S3);
             }
-            const double err = (S5 == 0.0 && S3 == 0.0) ? 0.0 : h_try * S5 / sqrt((S5 + 0.01 * S3) * (double)N);
+            const double err = (S5 == 0.0 && S3 == 0.0) ? 0.0 : h_try * S5 * fast_rsqrt((S5 + 0.01 * S3) * (double)N);
             if (err < 1.0) {
                 double factor = (err == 0.0) ? 10.0 : fmin(10.0, 0.9 * inv_root8(err));
                 if (rejected) factor = fmin(factor, 1.0);
