@@ -4,7 +4,6 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
-#include <vector>
 
 #include "../../include/chaoticus.h"
 #include "launch.h"

@@ -1,14 +1,21 @@
-// col_kernels.cuh -- "column layout" step kernels (CUDA path, sm_100a).
+// col_kernels.cuh -- "column layout" step kernels and the layout-generic run / LD kernels
+// (CUDA path, sm_100a).
 //
 // A trajectory's augmented state is 1 + K columns of n = 2 NDOF components: column 0 the orbit,
 // columns 1..K the deviation vectors.  The columns are dealt to a tile of L
 // consecutive lanes, CPL = ceil((1+K)/L) columns per lane:
-//   L = 1  : one trajectory per thread, everything in registers (Henon-Heiles, K <= 4);
-//   L > 1  : one column per lane (CPL = 1) for mid-size states (3-DoF Lyapunov spectrum:
-//            L = 8, lanes 0..6 busy); the orbit's stage coordinates are broadcast from lane 0
-//            by shuffle each stage, Gram-Schmidt broadcasts one column at a time.
+//   L = 1  : one trajectory per thread, everything in registers (Henon-Heiles, K <= 3);
+//   L > 1  : CPL columns per lane for mid-size states and for small ensembles (3-DoF Lyapunov
+//            spectrum: L = 4, CPL = 2; Henon-Heiles SALI up to 4096 trajectories: L = 4, CPL = 1);
+//            the orbit's stage coordinates are broadcast from lane 0 by shuffle each stage,
+//            Gram-Schmidt broadcasts one column at a time.
 // HBM layout is structure-of-arrays (include/chaoticus.h); it is touched once at the start
 // and once at the end of a call, everything in between runs out of registers.
+//
+// run_kernel<C, MODE, IND, ADAPT> and ld_kernel<C> are written against the per-lane state class C
+// of a layout (Col<Sys,K,L> here, Chain<NP,K> in chain_kernels.cuh): C::NI (q, p) pairs per lane,
+// C::L lanes per trajectory, load/store, force, do_renorm, indicator, finite_all, on_mask,
+// store_logs.
 #pragma once
 #include <cmath>
 #include "dop8_core.cuh"

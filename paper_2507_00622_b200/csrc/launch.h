@@ -40,9 +40,12 @@ int try_launch_hh_adapt2(const LaunchReq& rq);
 int try_launch_c3_more(const LaunchReq& rq);
 int try_launch_dp(const LaunchReq& rq);
 
+// Common front part of every launcher: when rq.info is set, report the launch shape of `kern` and
+// return 0 (or a CUDA error); otherwise return -2, meaning "go ahead and launch".
 template <class Kern>
 inline int finish_launch(const LaunchReq& rq, Kern kern, int tpb, int lanes, long long n_threads) {
     long long blocks = (n_threads + tpb - 1) / tpb;
+    if (blocks > 2147483647LL) return (int)cudaErrorInvalidConfiguration;  // gridDim.x limit
     if (rq.info) {
         cudaFuncAttributes at;
         cudaError_t e = cudaFuncGetAttributes(&at, kern);
