@@ -286,3 +286,42 @@ def test_double_pendulum_ld(chs, orc):
     f, b = chs.ld(DP, prm, dev(y0), 0.0, 0.01, 800)
     assert np.abs(f.cpu().numpy() / fo - 1).max() <= 1e-8 and np.abs(b.cpu().numpy() / bo - 1).max() <= 1e-8
     assert (fo > 0).all() and np.abs(fo - bo).max() > 1e-3        # the two directions really differ
+
+
+@pytest.mark.parametrize("n_ic", [1, 3])
+def test_tiny_ensembles_on_tile_layouts(chs, orc, n_ic):
+    """One or three trajectories: most tiles of the only warp are padding that shadows the last
+    trajectory (shuffles must stay convergent) and must not store anything."""
+    cfg = W.config("C5", n_ic=n_ic)
+    go = orc.gali(FPUT, cfg["params"], cfg["y"].copy(), cfg["w"].copy(), renorm_every=10, h=0.05, n_steps=300,
+                  precision="f80")["series"]
+    gg = chs.gali(FPUT, cfg["params"], dev(cfg["y"]), dev(cfg["w"]), renorm_every=10, h=0.05, n_steps=300)
+    assert np.abs(gg.cpu().numpy() / go - 1).max() <= 1e-8
+    cfg = W.config("C4", n_ic=n_ic)
+    lo = orc.lyap(C3, cfg["params"], cfg["y"].copy(), cfg["w"].copy(), renorm_every=10, h=0.01, n_steps=300,
+                  precision="f80")["lam"]
+    lg = chs.lyap(C3, cfg["params"], dev(cfg["y"]), dev(cfg["w"]), renorm_every=10, h=0.01, n_steps=300)
+    assert lam_err(lg.cpu().numpy(), lo, 3.0) <= 1e-8
+    cfg = W.config("C1", n_ic=1)   # 1 x 1 grid through the 4-lane SALI tile
+    so = orc.sali(HH, None, cfg["y"].copy(), cfg["w"].copy(), renorm_every=1, h=0.01, n_steps=300,
+                  precision="f80")["series"]
+    sg = chs.sali(HH, None, dev(cfg["y"]), dev(cfg["w"]), renorm_every=1, h=0.01, n_steps=300)
+    assert np.abs(sg.cpu().numpy() / so - 1).max() <= 1e-8
+
+
+def test_zero_length_runs(chs, orc):
+    """n_steps = 0 and t_end = t0: nothing is integrated; vectors come back (ortho)normalised, the
+    indicator is that of the entry vectors, lambda is NaN (no elapsed time), counters are zero."""
+    y0 = W.hh_grid(0.125, 5, 4)
+    w0 = W.deviation_vectors(20, 2, 4, 9, "raw")
+    for kw in (dict(h=0.01, n_steps=0), dict(adaptive=True, t_end=0.0, rtol=1e-9, atol=1e-9)):
+        yo, wo = y0.copy(), w0.copy()
+        so = orc.sali(HH, None, yo, wo, renorm_every=1, precision="f80", **kw)["series"]
+        yg, wg = dev(y0), dev(w0)
+        rep = chs.Report(20, "cuda")
+        sg = chs.sali(HH, None, yg, wg, renorm_every=1, report=rep, **kw).cpu().numpy()
+        assert np.abs(sg / so - 1).max() <= 1e-13
+        assert (yg.cpu().numpy() == y0).all() and np.abs(wg.cpu().numpy() - wo).max() <= 1e-15
+        assert (rep.n_accepted.cpu().numpy() == 0).all() and (rep.status.cpu().numpy() == 0).all()
+        lam = chs.lyap(HH, None, dev(y0), dev(w0), renorm_every=1, **kw).cpu().numpy()
+        assert np.isnan(lam).all()
