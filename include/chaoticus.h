@@ -163,6 +163,15 @@ int chaoticus_dfma_probe_mode(int mode, long long iters, int n_blocks, int n_thr
  * 1 sali, 2 gali, 3 ld, 4 lyap.  Returns CHS_EUNSUPPORTED if no kernel is compiled. */
 int chaoticus_kernel_info(const chs_problem* pb, int what, int k, int adaptive, long long n_ic, int* info5);
 
+/* Process-wide options.  "adaptive_refill" (1 = on, default; 0 = off): adaptive runs are launched as
+ * one resident wave of persistent tiles that take trajectories from a device work queue, so a lane
+ * (tile) whose trajectory has ended fetches the next one instead of idling until the slowest lane of
+ * its warp ends.  Same results per trajectory (each trajectory's arithmetic does not depend on which
+ * lane runs it: bit-identical outputs on and off).  Neutral on uniform ensembles, faster on ensembles
+ * with unequal step counts.  At most 64 adaptive calls may be in flight at once while it is
+ * on.  Off: one trajectory per tile, the grid covers the ensemble.  Returns CHS_EINVAL for an unknown name. */
+int chaoticus_set_option(const char* name, int value);
+
 const char* chaoticus_last_error(void); /* thread-local, static storage */
 int chaoticus_version(void);
 

@@ -25,7 +25,7 @@ EXPORTS = [
     "chaoticus_integrate_fixed", "chaoticus_integrate_adaptive", "chaoticus_sali", "chaoticus_gali",
     "chaoticus_ld", "chaoticus_lyap", "chaoticus_ld_host", "chaoticus_sali_host", "chaoticus_gali_host",
     "chaoticus_lyap_host", "chaoticus_integrate_host", "chaoticus_dfma_probe", "chaoticus_dfma_probe_mode",
-    "chaoticus_kernel_info",
+    "chaoticus_kernel_info", "chaoticus_set_option",
 ]
 
 
@@ -73,6 +73,7 @@ def _load():
     lib.chaoticus_dfma_probe.argtypes = [ll, i, i, vp, vp]
     lib.chaoticus_dfma_probe_mode.argtypes = [i, ll, i, i, vp, vp]
     lib.chaoticus_kernel_info.argtypes = [PP, i, i, i, ll, C.POINTER(C.c_int)]
+    lib.chaoticus_set_option.argtypes = [C.c_char_p, i]
     return lib
 
 
@@ -271,6 +272,11 @@ def integrate_host(system, params, y, **stepper):
     n = _dim(pb)
     st = _stepper(**stepper)
     _check(_lib.chaoticus_integrate_host(C.byref(pb), y.shape[1], _host(y, (n, y.shape[1]), "y"), C.byref(st), None))
+
+
+def set_option(name, value):
+    """Process-wide library option (include/chaoticus.h chaoticus_set_option), e.g. ("adaptive_refill", 1)."""
+    _check(_lib.chaoticus_set_option(name.encode(), int(value)))
 
 
 # ---- measurement aids --------------------------------------------------------------------------

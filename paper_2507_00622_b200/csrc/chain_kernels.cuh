@@ -35,6 +35,10 @@ struct Chain {
 #pragma unroll
         for (int j = 0; j < NCOL; j++) logacc_init(lg[j]);
     }
+    __device__ __forceinline__ void reset_logs() {
+#pragma unroll
+        for (int j = 0; j < NCOL; j++) logacc_init(lg[j]);
+    }
     __device__ __forceinline__ void load(const double* y, const double* w, long long n_ic, long long ic,
                                          double psign) {
         q[0] = y[(long long)lt * n_ic + ic];

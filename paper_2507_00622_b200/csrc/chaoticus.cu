@@ -8,9 +8,26 @@
 #include "../../include/chaoticus.h"
 #include "launch.h"
 
+#include <atomic>
+
 namespace {
 
 thread_local char g_err[512] = "";
+
+// lane refill of the adaptive kernels: option + a small pool of device work
+// counters, one per call in flight (a call zeroes its counter on its own stream before the launch)
+std::atomic<int> g_adaptive_refill{1};
+std::atomic<unsigned> g_queue_next{0};
+constexpr unsigned kQueueSlots = 64;
+__device__ unsigned long long g_queue_pool[kQueueSlots];
+
+unsigned long long* acquire_queue(cudaStream_t stream) {
+    unsigned long long* base = nullptr;
+    if (cudaGetSymbolAddress((void**)&base, g_queue_pool) != cudaSuccess) return nullptr;
+    unsigned long long* q = base + (g_queue_next.fetch_add(1) % kQueueSlots);
+    if (cudaMemsetAsync(q, 0, sizeof(unsigned long long), stream) != cudaSuccess) return nullptr;
+    return q;
+}
 
 int fail(int rc, const char* fmt, ...) {
     va_list ap;
@@ -164,6 +181,10 @@ int run_common(int what, const chs_problem* pb, long long n_ic, double* y, doubl
         a.t_final = rep->t_final;
     }
     if (n_ic == 0 && !info) return CHS_OK;
+    if (st->adaptive && !info && g_adaptive_refill.load() != 0 && pb->system != CHS_SYS_DOUBLE_PENDULUM) {
+        a.queue = acquire_queue(rq.stream);
+        if (!a.queue) return fail(CHS_ECUDA, "could not set up the lane-refill work queue");
+    }
     return finish(dispatch(rq), rq);
 }
 
@@ -172,6 +193,14 @@ int run_common(int what, const chs_problem* pb, long long n_ic, double* y, doubl
 extern "C" {
 
 int chaoticus_version(void) { return CHAOTICUS_VERSION; }
+
+int chaoticus_set_option(const char* name, int value) {
+    if (name && std::strcmp(name, "adaptive_refill") == 0) {
+        g_adaptive_refill.store(value != 0 ? 1 : 0);
+        return CHS_OK;
+    }
+    return fail(CHS_EINVAL, "unknown option '%s'", name ? name : "(null)");
+}
 const char* chaoticus_last_error(void) { return g_err; }
 
 int chaoticus_dim(const chs_problem* pb) { return dim_of(pb, nullptr); }

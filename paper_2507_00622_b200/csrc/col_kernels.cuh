@@ -52,6 +52,8 @@ struct RunArgs {
     const double* y0;
     double* ld_fwd;
     double* ld_bwd;
+    // adaptive runs: work queue for lane refill (device counter, zeroed before the launch), or null
+    unsigned long long* queue;
 };
 
 // one-sided (Hestenes) Jacobi on k columns of n components held by ONE thread; returns the
@@ -127,6 +129,11 @@ struct Col {
         prm = P;
         lt = (L == 1) ? 0 : (int)(threadIdx.x % L);
         s_lane = (L > 1 && lt == 0) ? 0.5 : 1.0;
+#pragma unroll
+        for (int j = 0; j < CPL; j++) logacc_init(lg[j]);
+    }
+
+    __device__ __forceinline__ void reset_logs() {
 #pragma unroll
         for (int j = 0; j < CPL; j++) logacc_init(lg[j]);
     }
@@ -421,28 +428,28 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
     constexpr int NI = C::NI, L = C::L, K = C::K;
     const long long gt = (long long)blockIdx.x * TPB + threadIdx.x;
     const long long traj = gt / L;
-    const bool valid = traj < a.n_ic;
-    const long long ic = valid ? traj : a.n_ic - 1;  // padding lanes shadow the last trajectory
+    const bool want_log = (a.logacc != nullptr) || (a.lambda != nullptr);
 
     C s;
     s.init(prm);
-    s.load(a.y, a.w, a.n_ic, ic, 1.0);
-    const bool want_log = (a.logacc != nullptr) || (a.lambda != nullptr);
-    s.template do_renorm<MODE>(false, true);  // on entry: no log accumulated
-
     const ForceFn<C> force{s};
     const NoHook nohook{};
 
     long long n_acc = 0, n_rej = 0;
     int status = ST_OK;
     double t = a.t0;
-    long long slot = 0;
     constexpr int NC = C::NCOMP > 0 ? C::NCOMP : 1;
     double qc[NC], pc[NC], qcn[NC], pcn[NC];  // carried rounding errors of the orbit update
 #pragma unroll
     for (int c = 0; c < NC; c++) qc[c] = pc[c] = 0.0;
 
     if constexpr (!ADAPT) {
+        // ---- fixed step: one trajectory per tile, every tile runs the same number of steps -------
+        const bool valid = traj < a.n_ic;
+        const long long ic = valid ? traj : a.n_ic - 1;  // padding tiles shadow the last trajectory
+        s.load(a.y, a.w, a.n_ic, ic, 1.0);
+        s.template do_renorm<MODE>(false, true);  // on entry: no log accumulated
+        long long slot = 0;
         int cd = a.m, sd = a.sample_every;
         for (long long st = 1; st <= a.n_steps; ++st) {
             double F[12][NI];
@@ -478,18 +485,73 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
         }
         n_acc = a.n_steps;
         t = a.t0 + (double)a.n_steps * a.h;
+        const bool bad = !s.finite_all();
+        if (bad) status = ST_NONFINITE;
+        double ind = 0.0;
+        if constexpr (IND != IND_NONE) ind = s.template indicator<IND>();
+        if (!valid) return;
+        s.store(a.y, a.w, a.n_ic, ic, bad);
+        if constexpr (K > 0) s.store_logs(a, ic, bad, t - a.t0);
+        if (s.lt == 0) {
+            if constexpr (IND != IND_NONE) {
+                if (a.series) {
+                    a.series[(a.n_samples - 1) * a.n_ic + ic] = bad ? nan("") : ind;
+                    if (bad)
+                        for (long long r = slot; r < a.n_samples - 1; r++) a.series[r * a.n_ic + ic] = nan("");
+                }
+            }
+            if (a.n_acc) a.n_acc[ic] = n_acc;
+            if (a.n_rej) a.n_rej[ic] = n_rej;
+            if (a.status) a.status[ic] = status;
+            if (a.t_final) a.t_final[ic] = t;
+        }
     } else {
+        // ---- adaptive step: every trajectory owns t, h, counters, status.
+        // A tile keeps taking trajectories until none is left: with a.queue set, from a global work
+        // queue (lane refill: a tile whose trajectory has ended fetches the next one instead of idling
+        // until the slowest lane of its warp and block ends; the grid is then one resident wave);
+        // without it, exactly one trajectory per tile.  The warp-wide loop and every section that
+        // shuffles stay convergent; per-tile decisions are predicates.
         const double dir = (a.t_end >= a.t0) ? 1.0 : -1.0;
-        double h_abs = a.h0 > 0.0 ? a.h0 : initial_step(s, fabs(a.t_end - a.t0), dir, a.rtol, a.atol);
-        long long attempts = 0;
-        bool rejected = false;
-        double min_step = 0.0;
-        int cd = a.m;
+        const double interval = fabs(a.t_end - a.t0);
         bool on[NI];
         s.on_mask(on);
+        double h_abs = 0.0, min_step = 0.0;
+        long long attempts = 0, ic = 0;
+        bool rejected = false, need = true, done = false, first_fetch = true;
+        int cd = a.m;
         while (true) {
-            bool active = valid && status == ST_OK && dir * (a.t_end - t) > 0.0;
-            if (!__any_sync(0xffffffffu, active)) break;
+            if (__any_sync(0xffffffffu, need)) {
+                long long nxt = a.n_ic;  // "nothing left"
+                if (a.queue != nullptr) {
+                    if (need && s.lt == 0) nxt = (long long)atomicAdd(a.queue, 1ULL);
+                    nxt = tile_bcast_ll<L>(nxt, 0);
+                } else if (first_fetch) {
+                    nxt = traj;
+                }
+                first_fetch = false;
+                const bool got = need && nxt < a.n_ic;
+                if (need && !got) done = true;
+                if (got) {
+                    ic = nxt;
+                    s.load(a.y, a.w, a.n_ic, ic, 1.0);
+                    s.reset_logs();
+                    t = a.t0;
+                    n_acc = n_rej = attempts = 0;
+                    status = ST_OK;
+                    rejected = false;
+                    cd = a.m;
+#pragma unroll
+                    for (int c = 0; c < NC; c++) qc[c] = pc[c] = 0.0;
+                }
+                s.template do_renorm<MODE>(false, got);  // on entry: no log accumulated
+                const double h_init = a.h0 > 0.0 ? a.h0 : initial_step(s, interval, dir, a.rtol, a.atol);
+                if (got) h_abs = h_init;
+                need = false;
+            }
+            if (!__any_sync(0xffffffffu, !done)) break;
+
+            bool active = !done && status == ST_OK && dir * (a.t_end - t) > 0.0;
             if (!rejected) {
                 min_step = 10.0 * fabs(nextafter(t, dir * INFINITY) - t);
                 h_abs = fmax(h_abs, min_step);
@@ -547,37 +609,38 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
                     rejected = true;
                     n_rej++;
                 } else {
+                    // inf or NaN in y+ makes its error scale, hence err, NaN (fast_rcp(inf) is NaN)
                     status = ST_NONFINITE;
                 }
             }
             if constexpr (MODE != MODE_NONE) {
                 if (__any_sync(0xffffffffu, ren)) s.template do_renorm<MODE>(want_log, ren);
             }
-            // a non-finite y+ needs no separate test here: inf or NaN in y+ makes its error scale, hence
-            // err, NaN (fast_rcp(inf) is NaN), which the branch above turns into ST_NONFINITE
-        }
-    }
-    // ---- outputs ------------------------------------------------------------------------------
-    bool bad = !s.finite_all();
-    if (ADAPT) bad = tile_any<L>(status != ST_OK) || bad;
-    if (bad && status == ST_OK) status = ST_NONFINITE;
-    double ind = 0.0;
-    if constexpr (IND != IND_NONE) ind = s.template indicator<IND>();
-    if (!valid) return;
-    s.store(a.y, a.w, a.n_ic, ic, bad);
-    if constexpr (K > 0) s.store_logs(a, ic, bad, t - a.t0);
-    if (s.lt == 0) {
-        if constexpr (IND != IND_NONE) {
-            if (a.series) {
-                a.series[(a.n_samples - 1) * a.n_ic + ic] = bad ? nan("") : ind;
-                if (bad)
-                    for (long long r = slot; r < a.n_samples - 1; r++) a.series[r * a.n_ic + ic] = nan("");
+
+            // trajectories that ended in this iteration: write their results, ask for the next one
+            const bool fin = !done && !(status == ST_OK && dir * (a.t_end - t) > 0.0);
+            if (__any_sync(0xffffffffu, fin)) {
+                bool bad = !s.finite_all();
+                bad = tile_any<L>(status != ST_OK) || bad;
+                double ind = 0.0;
+                if constexpr (IND != IND_NONE) ind = s.template indicator<IND>();
+                if (fin) {
+                    const int st_out = (bad && status == ST_OK) ? (int)ST_NONFINITE : status;
+                    s.store(a.y, a.w, a.n_ic, ic, bad);
+                    if constexpr (K > 0) s.store_logs(a, ic, bad, t - a.t0);
+                    if (s.lt == 0) {
+                        if constexpr (IND != IND_NONE) {
+                            if (a.series) a.series[ic] = bad ? nan("") : ind;  // adaptive: n_samples = 1
+                        }
+                        if (a.n_acc) a.n_acc[ic] = n_acc;
+                        if (a.n_rej) a.n_rej[ic] = n_rej;
+                        if (a.status) a.status[ic] = st_out;
+                        if (a.t_final) a.t_final[ic] = t;
+                    }
+                    need = true;
+                }
             }
         }
-        if (a.n_acc) a.n_acc[ic] = n_acc;
-        if (a.n_rej) a.n_rej[ic] = n_rej;
-        if (a.status) a.status[ic] = status;
-        if (a.t_final) a.t_final[ic] = t;
     }
 }
 

@@ -49,6 +49,11 @@ __device__ __forceinline__ double tile_bcast(double x, int src_lane_in_tile) {
     else return __shfl_sync(0xffffffffu, x, src_lane_in_tile, L);
 }
 template <int L>
+__device__ __forceinline__ long long tile_bcast_ll(long long x, int src_lane_in_tile) {
+    if constexpr (L == 1) return x;
+    else return __shfl_sync(0xffffffffu, x, src_lane_in_tile, L);
+}
+template <int L>
 __device__ __forceinline__ double tile_sum(double x) {  // butterfly: identical on all lanes
     if constexpr (L > 1) {
 #pragma unroll

@@ -16,7 +16,7 @@ int run_chain(const LaunchReq& rq) {
     const long long n_threads = rq.args.n_ic * NP;
     int r = finish_launch(rq, kern, TPB, NP, n_threads);
     if (r != -2) return r;
-    const long long blocks = (n_threads + TPB - 1) / TPB;
+    const long long blocks = run_grid(rq, kern, TPB, n_threads);
     if (blocks == 0) return 0;
     kern<<<(unsigned)blocks, TPB, 0, rq.stream>>>(rq.tab, prm, rq.args);
     return (int)cudaGetLastError();

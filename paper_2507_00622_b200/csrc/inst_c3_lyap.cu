@@ -4,7 +4,7 @@
 namespace chs {
 int try_launch_c3_lyap(const LaunchReq& rq) {
     if (CHS_MATCH(1, WHAT_LYAP, 6, 0)) return run_col<Coupled3, 6, 4, MODE_MGS, IND_NONE, false, 128, 2>(rq);
-    if (CHS_MATCH(1, WHAT_LYAP, 6, 1)) return run_col<Coupled3, 6, 8, MODE_MGS, IND_NONE, true, 128, 3>(rq);
+    if (CHS_MATCH(1, WHAT_LYAP, 6, 1)) return run_col<Coupled3, 6, 8, MODE_MGS, IND_NONE, true, 128, 2>(rq);
     if (CHS_MATCH(1, WHAT_GALI, 2, 0)) return run_col<Coupled3, 2, 4, MODE_NORM, IND_GALI, false, 128, 4>(rq);
     if (CHS_MATCH(1, WHAT_GALI, 3, 0)) return run_col<Coupled3, 3, 4, MODE_NORM, IND_GALI, false, 128, 4>(rq);
     return -1;

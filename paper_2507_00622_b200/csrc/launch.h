@@ -56,6 +56,26 @@ inline int finish_launch(const LaunchReq& rq, Kern kern, int tpb, int lanes, lon
     return -2;  // caller launches
 }
 
+// blocks of one resident wave of `kern` (lane-refill launches are persistent: DESIGN.md "Adaptive")
+template <class Kern>
+inline long long resident_blocks(Kern kern, int tpb) {
+    int dev = 0, sms = 0, nb = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, tpb, 0);
+    return (long long)sms * (nb > 0 ? nb : 1);
+}
+// grid of a run_kernel launch: the whole ensemble, or one resident wave when a work queue is attached
+template <class Kern>
+inline long long run_grid(const LaunchReq& rq, Kern kern, int tpb, long long n_threads) {
+    long long blocks = (n_threads + tpb - 1) / tpb;
+    if (rq.adaptive && rq.args.queue != nullptr) {
+        const long long res = resident_blocks(kern, tpb);
+        if (res < blocks) blocks = res;
+    }
+    return blocks;
+}
+
 template <class Sys, int K, int L, int MODE, int IND, bool ADAPT, int TPB, int MINB>
 inline int run_col(const LaunchReq& rq) {
     typename Sys::Params prm;
@@ -64,7 +84,7 @@ inline int run_col(const LaunchReq& rq) {
     const long long n_threads = rq.args.n_ic * L;
     int r = finish_launch(rq, kern, TPB, L, n_threads);
     if (r != -2) return r;
-    const long long blocks = (n_threads + TPB - 1) / TPB;
+    const long long blocks = run_grid(rq, kern, TPB, n_threads);
     if (blocks == 0) return 0;
     kern<<<(unsigned)blocks, TPB, 0, rq.stream>>>(rq.tab, prm, rq.args);
     return (int)cudaGetLastError();

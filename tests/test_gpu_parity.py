@@ -486,3 +486,33 @@ def test_adaptive_escaping_orbit_status(chs):
     ok = np.delete(np.arange(25), 7)
     assert (st[ok] == 0).all() and np.isfinite(out[:, ok]).all()
     assert (rep.t_final.cpu().numpy()[ok] == 200.0).all()
+
+
+def test_adaptive_lane_refill_is_result_neutral(chs):
+    """Lane refill (persistent tiles + device work queue) changes which lane runs a trajectory,
+    never its arithmetic: outputs are bit-identical with the option on and off, on a deliberately
+    unequal ensemble (E = 1/6 orbits interleaved with E = 0.01 orbits that need far fewer steps)
+    for the thread layout and for a tile layout."""
+    import torch
+    ya, yb = W.hh_grid(1.0 / 6.0, 40, 25), W.hh_grid(0.01, 40, 25)
+    y0 = np.empty((4, 2000))
+    y0[:, 0::2], y0[:, 1::2] = ya, yb
+    w0 = W.deviation_vectors(2000, 2, 4, 0, "unit")
+    cfg = W.config("C5", n_ic=300)
+    outs = {}
+    try:
+        for mode in (0, 1):
+            chs.set_option("adaptive_refill", mode)
+            yg, wg, rep = dev(y0), dev(w0), chs.Report(2000, "cuda")
+            s = chs.sali(HH, None, yg, wg, renorm_every=1, adaptive=True, t_end=150.0, rtol=1e-11, atol=1e-11, report=rep)
+            fy, fw = dev(cfg["y"]), dev(cfg["w"])
+            g = chs.gali(FPUT, cfg["params"], fy, fw, renorm_every=2, adaptive=True, t_end=40.0, rtol=1e-8, atol=1e-8)
+            outs[mode] = [t.clone() for t in (s, yg, wg, rep.n_accepted, rep.n_rejected, rep.t_final, g, fy, fw)]
+    finally:
+        chs.set_option("adaptive_refill", 1)
+    for a, b in zip(outs[0], outs[1]):
+        assert torch.equal(a, b)
+    acc = outs[1][3].cpu().numpy()
+    assert acc.max() > 1.3 * acc.min()      # the ensemble really is unequal
+    with pytest.raises(chs.ChaoticusError):
+        chs.set_option("no_such_option", 1)
