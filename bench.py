@@ -332,11 +332,12 @@ def main():
         return ms
 
     # FP64 FMA peak of this device, measured live (register-only DFMA chains)
-    chs.dfma_probe(1000, 148 * 8)
+    from paper_2507_00622_b200 import probe
+    probe.dfma_probe(1000, 148 * 8)
     torch.cuda.synchronize()
     pe0, pe1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     pe0.record()
-    probe_flop, _ = chs.dfma_probe(400000, 148 * 8)
+    probe_flop, _ = probe.dfma_probe(400000, 148 * 8)
     pe1.record()
     torch.cuda.synchronize()
     dfma_tflops = probe_flop / (pe0.elapsed_time(pe1) * 1e-3) / 1e12

@@ -35,7 +35,7 @@
 extern "C" {
 #endif
 
-#define CHAOTICUS_VERSION 100 /* 0.1.0 */
+#define CHAOTICUS_VERSION 200 /* 0.2.0 */
 
 typedef enum { CHS_OK = 0, CHS_EINVAL = 1, CHS_EUNSUPPORTED = 2, CHS_ECUDA = 3 } chs_rc;
 
@@ -75,16 +75,30 @@ typedef struct {
     long long max_steps;          /* adaptive */
 } chs_stepper;
 
-/* Per-trajectory report; every member is DEVICE [n_ic] or NULL. */
+/* Per-trajectory report and continuation state; the array members are DEVICE or NULL.
+ * Checkpoint / resume: y and w are advanced in place, so a second call
+ * continues the run.  The orbit is advanced with a compensated sum whose carried rounding word
+ * lives in registers; `carry` takes it across a call boundary.  A
+ * continuation call (resume = 1) reads `carry` on entry and does NOT normalise / orthonormalise
+ * w on entry (w is the unit / orthonormal set the previous call returned).  With carry and
+ * resume = 1, a fixed-step run split at a multiple of renorm_every steps gives y, w and the
+ * indicator BIT-IDENTICAL to the one-call run (lognorm / logsum / lambda agree to rounding only:
+ * the logarithm of a product is taken once per call).  Adaptive runs of the separable systems
+ * honour resume (no entry normalisation) but neither read nor write carry: their last step is
+ * clipped to t_end, so a split adaptive run is a different step sequence anyway. */
 #define CHS_ST_OK 0
 #define CHS_ST_NONFINITE 1
 #define CHS_ST_UNDERFLOW 2
 #define CHS_ST_MAXSTEPS 3
 typedef struct {
-    long long* n_accepted; /* accepted steps (fixed: n_steps) */
-    long long* n_rejected; /* rejected attempts (fixed: 0) */
-    int* status;           /* CHS_ST_* */
-    double* t_final;       /* time reached */
+    long long* n_accepted; /* [n_ic] accepted steps (fixed: n_steps) */
+    long long* n_rejected; /* [n_ic] rejected attempts (fixed: 0) */
+    int* status;           /* [n_ic] CHS_ST_* */
+    double* t_final;       /* [n_ic] time reached */
+    double* carry;         /* [n][n_ic] (layout of y) in/out: carried rounding words of the orbit
+                              update; written at the end of every run, read on entry iff resume */
+    int resume;            /* 0: fresh run (carry starts at 0, w normalised on entry);
+                              1: continuation of a previous call (see above) */
 } chs_report;
 
 /* phase-space dimension n of a problem, or -1 */
@@ -128,7 +142,8 @@ int chaoticus_ld(const chs_problem* pb, long long n_ic, const double* y0, double
 
 /* PAPER.md:51-52 (solvers 5, 6): 1 <= k <= n vectors, modified Gram-Schmidt every
  * renorm_every accepted steps and at the end (orthonormalised once on entry),
- * S_v += ln r_vv.  lambda DEVICE [k][n_ic] = this run's sums / elapsed time (may be NULL);
+ * S_v += ln r_vv.  lambda DEVICE [k][n_ic] = this run's sums / |elapsed time| (growth rates per
+ * unit of |t|, also for backward-time runs: DESIGN.md R18; may be NULL);
  * logsum DEVICE [k][n_ic] or NULL: the run ADDS its sums. */
 int chaoticus_lyap(const chs_problem* pb, long long n_ic, double* y, double* w, int k, const chs_stepper* st,
                    int renorm_every, double* lambda, double* logsum, const chs_report* rep, void* stream);
@@ -149,15 +164,6 @@ int chaoticus_lyap_host(const chs_problem* pb, long long n_ic, double* y, double
 int chaoticus_integrate_host(const chs_problem* pb, long long n_ic, double* y, const chs_stepper* st,
                              const chs_report* rep);
 
-/* Measurement aid: a register-only chain of dependent-free DFMAs,
- * n_blocks x n_threads threads x iters x 16 DFMA each; out DEVICE [n_blocks*n_threads]
- * (keeps the work alive).  Used by bench.py to measure the FP64 FMA peak of the device. */
-int chaoticus_dfma_probe(long long iters, int n_blocks, int n_threads, double* out, void* stream);
-/* Variants of the probe: mode 0 as above (fixed register operands); mode 1: the multiplier comes
- * from the constant bank, as the step kernels read the tableau; mode 2: three distinct register
- * operands per DFMA (register-file bandwidth included). */
-int chaoticus_dfma_probe_mode(int mode, long long iters, int n_blocks, int n_threads, double* out, void* stream);
-
 /* Kernel launch shape the library would use for a call (for reporting): writes threads per
  * block, blocks, lanes per trajectory, registers per thread, spill bytes.  what: 0 integrate,
  * 1 sali, 2 gali, 3 ld, 4 lyap.  Returns CHS_EUNSUPPORTED if no kernel is compiled. */
@@ -168,8 +174,9 @@ int chaoticus_kernel_info(const chs_problem* pb, int what, int k, int adaptive, 
  * (tile) whose trajectory has ended fetches the next one instead of idling until the slowest lane of
  * its warp ends.  Same results per trajectory (each trajectory's arithmetic does not depend on which
  * lane runs it: bit-identical outputs on and off).  Neutral on uniform ensembles, faster on ensembles
- * with unequal step counts.  At most 64 adaptive calls may be in flight at once while it is
- * on.  Off: one trajectory per tile, the grid covers the ensemble.  Returns CHS_EINVAL for an unknown name. */
+ * with unequal step counts.  Each call in flight owns one of 64 device work counters per
+ * device (tracked by an event recorded after its launch); when all 64 are busy the call is launched
+ * without refill instead (same results).  Off: one trajectory per tile, the grid covers the ensemble.  Returns CHS_EINVAL for an unknown name. */
 int chaoticus_set_option(const char* name, int value);
 
 const char* chaoticus_last_error(void); /* thread-local, static storage */

@@ -665,7 +665,8 @@ static void scatter(long long n_ic, long long ic, int n, int k, const real *Y, d
 /* General run.  y [n][n_ic] in/out; w [k][n][n_ic] in/out (k may be 0, w NULL).
  * series [n_samples][n_ic] or NULL; logacc [k][n_ic] in/out accumulators or NULL (the run
  * ADDS its sum of ln(alpha_v) resp. ln(r_vv)); lambda [k][n_ic] or NULL = this run's sums
- * divided by this run's elapsed time.  Report arrays may be NULL. */
+ * divided by the LENGTH |t_final - t0| of this run's time interval (R18: an exponent
+ * is a growth rate per unit of elapsed |t|, also for backward-time runs).  Report arrays may be NULL. */
 int orc_run(int sys, const double *params, long long n_ic, double *y, double *w, int k, int adaptive,
             double t0, double h, long long n_steps, double t_end, double rtol, double atol, double h0,
             long long max_steps, int mode, int indicator, int renorm_every, int sample_every,
@@ -712,7 +713,7 @@ int orc_run(int sys, const double *params, long long n_ic, double *y, double *w,
             real elapsed = rep.t_final - st.t0;
             for (int v = 0; v < k; v++) {
                 if (logacc) logacc[(long long)v * n_ic + ic] = bad ? NAN : logacc[(long long)v * n_ic + ic] + (double)L[v];
-                if (lambda) lambda[(long long)v * n_ic + ic] = (bad || elapsed == 0) ? NAN : (double)(L[v] / elapsed);
+                if (lambda) lambda[(long long)v * n_ic + ic] = (bad || elapsed == 0) ? NAN : (double)(L[v] / R_FABS(elapsed));
             }
             if (n_acc) n_acc[ic] = rep.n_acc;
             if (n_rej) n_rej[ic] = rep.n_rej;

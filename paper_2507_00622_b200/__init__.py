@@ -9,7 +9,7 @@ indicators (the hot path of arXiv 2507.00622).
 import importlib
 
 _API = ("integrate_fixed", "integrate_adaptive", "sali", "gali", "ld", "lyap", "ld_host", "sali_host", "gali_host",
-        "lyap_host", "integrate_host", "Report", "kernel_info", "dfma_probe", "dim", "n_samples", "version", "set_option")
+        "lyap_host", "integrate_host", "Report", "HostReport", "kernel_info", "dim", "n_samples", "version", "set_option")
 
 
 def __getattr__(name):

@@ -24,8 +24,7 @@ EXPORTS = [
     "chaoticus_version", "chaoticus_last_error", "chaoticus_dim", "chaoticus_n_samples",
     "chaoticus_integrate_fixed", "chaoticus_integrate_adaptive", "chaoticus_sali", "chaoticus_gali",
     "chaoticus_ld", "chaoticus_lyap", "chaoticus_ld_host", "chaoticus_sali_host", "chaoticus_gali_host",
-    "chaoticus_lyap_host", "chaoticus_integrate_host", "chaoticus_dfma_probe", "chaoticus_dfma_probe_mode",
-    "chaoticus_kernel_info", "chaoticus_set_option",
+    "chaoticus_lyap_host", "chaoticus_integrate_host", "chaoticus_kernel_info", "chaoticus_set_option",
 ]
 
 
@@ -45,7 +44,7 @@ class _Stepper(C.Structure):
 
 class _Report(C.Structure):
     _fields_ = [("n_accepted", C.c_void_p), ("n_rejected", C.c_void_p), ("status", C.c_void_p),
-                ("t_final", C.c_void_p)]
+                ("t_final", C.c_void_p), ("carry", C.c_void_p), ("resume", C.c_int)]
 
 
 def _load():
@@ -70,8 +69,6 @@ def _load():
     lib.chaoticus_gali_host.argtypes = [PP, ll, vp, vp, i, SP, i, i, vp, vp, RP]
     lib.chaoticus_lyap_host.argtypes = [PP, ll, vp, vp, i, SP, i, vp, vp, RP]
     lib.chaoticus_integrate_host.argtypes = [PP, ll, vp, SP, RP]
-    lib.chaoticus_dfma_probe.argtypes = [ll, i, i, vp, vp]
-    lib.chaoticus_dfma_probe_mode.argtypes = [i, ll, i, i, vp, vp]
     lib.chaoticus_kernel_info.argtypes = [PP, i, i, i, ll, C.POINTER(C.c_int)]
     lib.chaoticus_set_option.argtypes = [C.c_char_p, i]
     return lib
@@ -130,19 +127,47 @@ def _stream():
 
 
 class Report:
-    """Per-trajectory report arrays (device tensors)."""
+    """Per-trajectory report arrays (device tensors) and continuation state (chs_report).
 
-    def __init__(self, n_ic, device):
+    n: phase-space dimension; if given, a `carry` tensor [n, n_ic] is attached (the carried
+    rounding words of the orbit update).  Set `resume = True` before a continuation call."""
+
+    def __init__(self, n_ic, device, n=None):
         self.n_accepted = torch.zeros(n_ic, dtype=torch.int64, device=device)
         self.n_rejected = torch.zeros(n_ic, dtype=torch.int64, device=device)
         self.status = torch.zeros(n_ic, dtype=torch.int32, device=device)
         self.t_final = torch.zeros(n_ic, dtype=torch.float64, device=device)
-        self._c = _Report(self.n_accepted.data_ptr(), self.n_rejected.data_ptr(), self.status.data_ptr(),
-                          self.t_final.data_ptr())
+        self.carry = torch.zeros((n, n_ic), dtype=torch.float64, device=device) if n else None
+        self.resume = False
+
+    def _struct(self):
+        return _Report(self.n_accepted.data_ptr(), self.n_rejected.data_ptr(), self.status.data_ptr(),
+                       self.t_final.data_ptr(), self.carry.data_ptr() if self.carry is not None else None,
+                       int(bool(self.resume)))
+
+
+class HostReport:
+    """As Report, with host (numpy) arrays, for the *_host entry points."""
+
+    def __init__(self, n_ic, n=None):
+        self.n_accepted = np.zeros(n_ic, dtype=np.int64)
+        self.n_rejected = np.zeros(n_ic, dtype=np.int64)
+        self.status = np.zeros(n_ic, dtype=np.int32)
+        self.t_final = np.zeros(n_ic)
+        self.carry = np.zeros((n, n_ic)) if n else None
+        self.resume = False
+
+    def _struct(self):
+        return _Report(self.n_accepted.ctypes.data, self.n_rejected.ctypes.data, self.status.ctypes.data,
+                       self.t_final.ctypes.data, self.carry.ctypes.data if self.carry is not None else None,
+                       int(bool(self.resume)))
 
 
 def _rep(report):
-    return C.byref(report._c) if report is not None else None
+    if report is None:
+        return None
+    report._c = report._struct()   # kept alive on the object for the duration of the call
+    return C.byref(report._c)
 
 
 # ---- the six entry points (same names as the C ABI, without the prefix) ----------------------
@@ -235,7 +260,8 @@ def ld_host(system, params, y0, t0, h, n_steps, ld_fwd=None, ld_bwd=None):
                                   _host(ld_fwd, (n_ic,), "ld_fwd"), _host(ld_bwd, (n_ic,), "ld_bwd")))
 
 
-def sali_host(system, params, y, w, sali_out, *, renorm_every=1, sample_every=0, lognorm=None, **stepper):
+def sali_host(system, params, y, w, sali_out, *, renorm_every=1, sample_every=0, lognorm=None, report=None,
+              **stepper):
     pb = _problem(system, params)
     n = _dim(pb)
     n_ic = y.shape[1]
@@ -243,10 +269,11 @@ def sali_host(system, params, y, w, sali_out, *, renorm_every=1, sample_every=0,
     ns = 1 if st.adaptive else n_samples(st.n_steps, renorm_every, sample_every)
     _check(_lib.chaoticus_sali_host(C.byref(pb), n_ic, _host(y, (n, n_ic), "y"), _host(w, (2, n, n_ic), "w"),
                                     C.byref(st), renorm_every, sample_every, _host(sali_out, (ns, n_ic), "sali"),
-                                    _host(lognorm, (2, n_ic), "lognorm"), None))
+                                    _host(lognorm, (2, n_ic), "lognorm"), _rep(report)))
 
 
-def gali_host(system, params, y, w, gali_out, *, renorm_every=1, sample_every=0, lognorm=None, **stepper):
+def gali_host(system, params, y, w, gali_out, *, renorm_every=1, sample_every=0, lognorm=None, report=None,
+              **stepper):
     pb = _problem(system, params)
     n = _dim(pb)
     n_ic, k = y.shape[1], w.shape[0]
@@ -254,24 +281,25 @@ def gali_host(system, params, y, w, gali_out, *, renorm_every=1, sample_every=0,
     ns = 1 if st.adaptive else n_samples(st.n_steps, renorm_every, sample_every)
     _check(_lib.chaoticus_gali_host(C.byref(pb), n_ic, _host(y, (n, n_ic), "y"), _host(w, (k, n, n_ic), "w"), k,
                                     C.byref(st), renorm_every, sample_every, _host(gali_out, (ns, n_ic), "gali"),
-                                    _host(lognorm, (k, n_ic), "lognorm"), None))
+                                    _host(lognorm, (k, n_ic), "lognorm"), _rep(report)))
 
 
-def lyap_host(system, params, y, w, lambda_out, *, renorm_every=1, logsum=None, **stepper):
+def lyap_host(system, params, y, w, lambda_out, *, renorm_every=1, logsum=None, report=None, **stepper):
     pb = _problem(system, params)
     n = _dim(pb)
     n_ic, k = y.shape[1], w.shape[0]
     st = _stepper(**stepper)
     _check(_lib.chaoticus_lyap_host(C.byref(pb), n_ic, _host(y, (n, n_ic), "y"), _host(w, (k, n, n_ic), "w"), k,
                                     C.byref(st), renorm_every, _host(lambda_out, (k, n_ic), "lambda"),
-                                    _host(logsum, (k, n_ic), "logsum"), None))
+                                    _host(logsum, (k, n_ic), "logsum"), _rep(report)))
 
 
-def integrate_host(system, params, y, **stepper):
+def integrate_host(system, params, y, report=None, **stepper):
     pb = _problem(system, params)
     n = _dim(pb)
     st = _stepper(**stepper)
-    _check(_lib.chaoticus_integrate_host(C.byref(pb), y.shape[1], _host(y, (n, y.shape[1]), "y"), C.byref(st), None))
+    _check(_lib.chaoticus_integrate_host(C.byref(pb), y.shape[1], _host(y, (n, y.shape[1]), "y"), C.byref(st),
+                                         _rep(report)))
 
 
 def set_option(name, value):
@@ -279,14 +307,7 @@ def set_option(name, value):
     _check(_lib.chaoticus_set_option(name.encode(), int(value)))
 
 
-# ---- measurement aids --------------------------------------------------------------------------
-def dfma_probe(iters, n_blocks, n_threads=256, mode=0):
-    """Launches the DFMA peak probe on the current stream; returns the FP64 flop it performs."""
-    out = torch.empty(n_blocks * n_threads, dtype=torch.float64, device="cuda")
-    _check(_lib.chaoticus_dfma_probe_mode(mode, int(iters), n_blocks, n_threads, out.data_ptr(), _stream()))
-    return 2.0 * 16.0 * iters * n_blocks * n_threads, out
-
-
+# ---- reporting ---------------------------------------------------------------------------------
 def kernel_info(system, params, what, k=0, adaptive=False, n_ic=1):
     """dict(tpb, blocks, lanes, regs, spill_bytes) of the kernel a call would launch."""
     pb = _problem(system, params)

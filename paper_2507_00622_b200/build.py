@@ -1,4 +1,5 @@
-"""Builds paper_2507_00622_b200/libchaoticus.so in-tree with nvcc for sm_100a.
+"""Builds paper_2507_00622_b200/libchaoticus.so (the product) and libchaoticus_probe.so (the
+bench-only DFMA peak probe) in-tree with nvcc for sm_100a.
 
     python -m paper_2507_00622_b200.build [--force]
 
@@ -14,7 +15,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 BUILD = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libchaoticus.so")
-UNITS = ["chaoticus", "probe", "inst_hh", "inst_hh_ind", "inst_hh_adapt", "inst_c3", "inst_c3_lyap", "inst_fput",
+PROBE_LIB = os.path.join(HERE, "libchaoticus_probe.so")
+UNITS = ["chaoticus", "inst_hh", "inst_hh_ind", "inst_hh_adapt", "inst_c3", "inst_c3_lyap", "inst_fput",
          "inst_fput_adapt", "inst_fput_n4", "inst_fput_n16", "inst_fput_n32", "inst_hh_adapt2", "inst_c3_more", "inst_dp"]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xptxas", "-v",
               "-Xcompiler", "-fPIC"]
@@ -40,14 +42,16 @@ def build(force=False, verbose=False):
     os.makedirs(BUILD, exist_ok=True)
     deps = _deps()
     newest = max(os.path.getmtime(d) for d in deps)
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
+    if (not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest and os.path.exists(PROBE_LIB)
+            and os.path.getmtime(PROBE_LIB) >= newest):
         return LIB
     with cf.ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
-        objs = list(ex.map(_compile, UNITS))
-    r = subprocess.run(["nvcc", "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB, *objs,
-                        "-lcudart"], capture_output=True, text=True)
-    if r.returncode != 0:
-        raise RuntimeError("link failed:\n" + r.stdout + r.stderr)
+        objs = list(ex.map(_compile, UNITS + ["probe"]))
+    for lib, members in ((LIB, objs[:-1]), (PROBE_LIB, objs[-1:])):
+        r = subprocess.run(["nvcc", "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", lib, *members,
+                            "-lcudart"], capture_output=True, text=True)
+        if r.returncode != 0:
+            raise RuntimeError("link failed:\n" + r.stdout + r.stderr)
     if verbose:
         print(spill_report())
     return LIB

@@ -65,9 +65,21 @@ struct Chain {
             const long long o = (long long)(v - 1) * a.n_ic + ic;
             const double lv = logacc_value(lg[v]);
             if (a.logacc) a.logacc[o] = bad ? nan("") : a.logacc[o] + lv;
-            if (a.lambda) a.lambda[o] = (bad || elapsed == 0.0) ? nan("") : lv / elapsed;
+            if (a.lambda) a.lambda[o] = (bad || elapsed == 0.0) ? nan("") : lv / fabs(elapsed);
         }
     }
+    // carried rounding word of this particle's orbit coordinate across a call boundary
+    __device__ __forceinline__ void load_carry(const double* cw, long long n_ic, long long ic, double (&qc)[1],
+                                               double (&pc)[1]) const {
+        qc[0] = cw[(long long)lt * n_ic + ic];
+        pc[0] = cw[(long long)(NP + lt) * n_ic + ic];
+    }
+    __device__ __forceinline__ void store_carry(double* cw, long long n_ic, long long ic, const double (&qc)[1],
+                                                const double (&pc)[1], bool bad) const {
+        cw[(long long)lt * n_ic + ic] = bad ? 0.0 : qc[0];
+        cw[(long long)(NP + lt) * n_ic + ic] = bad ? 0.0 : pc[0];
+    }
+    __device__ __forceinline__ void scrub_carry(double (&)[1], double (&)[1]) const {}
     __device__ __forceinline__ void on_mask(bool (&on)[NI]) const {
 #pragma unroll
         for (int c = 0; c < NI; c++) on[c] = true;

@@ -9,24 +9,77 @@
 #include "launch.h"
 
 #include <atomic>
+#include <mutex>
 
 namespace {
 
 thread_local char g_err[512] = "";
 
-// lane refill of the adaptive kernels: option + a small pool of device work
-// counters, one per call in flight (a call zeroes its counter on its own stream before the launch)
+// lane refill of the adaptive kernels: option + a pool of device work counters
+// per device.  A call in flight OWNS its counter: the slot keeps an event recorded on the call's stream
+// right after the kernel launch and is handed out again only once that event has completed.  When every
+// slot is busy the call runs without refill (one trajectory per tile: same results, bit for bit).
 std::atomic<int> g_adaptive_refill{1};
-std::atomic<unsigned> g_queue_next{0};
-constexpr unsigned kQueueSlots = 64;
-__device__ unsigned long long g_queue_pool[kQueueSlots];
+constexpr int kQueueSlots = 64, kMaxDevices = 64;
+struct QueuePool {
+    unsigned long long* base = nullptr;  // kQueueSlots device counters (cudaMalloc, never freed)
+    cudaEvent_t done[kQueueSlots] = {};
+    bool used[kQueueSlots] = {};
+    bool pending[kQueueSlots] = {};  // leased, kernel not launched yet: the event does not cover it
+};
+QueuePool g_pools[kMaxDevices];
+std::mutex g_pool_mutex;
 
-unsigned long long* acquire_queue(cudaStream_t stream) {
-    unsigned long long* base = nullptr;
-    if (cudaGetSymbolAddress((void**)&base, g_queue_pool) != cudaSuccess) return nullptr;
-    unsigned long long* q = base + (g_queue_next.fetch_add(1) % kQueueSlots);
-    if (cudaMemsetAsync(q, 0, sizeof(unsigned long long), stream) != cudaSuccess) return nullptr;
-    return q;
+struct QueueLease {
+    unsigned long long* counter = nullptr;
+    int dev = -1, slot = -1;
+};
+
+// a free counter of the current device, zeroed on `stream`; counter == nullptr: none free (or no device)
+QueueLease acquire_queue(cudaStream_t stream) {
+    QueueLease l;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return l;
+    std::lock_guard<std::mutex> lock(g_pool_mutex);
+    QueuePool& P = g_pools[dev];
+    if (!P.base && cudaMalloc((void**)&P.base, sizeof(unsigned long long) * kQueueSlots) != cudaSuccess) {
+        P.base = nullptr;
+        cudaGetLastError();
+        return l;
+    }
+    for (int s = 0; s < kQueueSlots; s++) {
+        if (P.used[s]) {
+            if (P.pending[s] || cudaEventQuery(P.done[s]) != cudaSuccess) {
+                cudaGetLastError();  // cudaErrorNotReady is not sticky, clear it
+                continue;
+            }
+            P.used[s] = false;
+        }
+        if (!P.done[s] && cudaEventCreateWithFlags(&P.done[s], cudaEventDisableTiming) != cudaSuccess) {
+            P.done[s] = nullptr;
+            cudaGetLastError();
+            return l;
+        }
+        if (cudaMemsetAsync(P.base + s, 0, sizeof(unsigned long long), stream) != cudaSuccess) return l;
+        P.used[s] = P.pending[s] = true;  // the event is recorded by release_after_launch
+        l.counter = P.base + s;
+        l.dev = dev;
+        l.slot = s;
+        return l;
+    }
+    return l;
+}
+// the slot becomes free when everything enqueued on `stream` so far (the kernel) has completed
+void release_after_launch(const QueueLease& l, cudaStream_t stream) {
+    if (l.slot < 0) return;
+    std::lock_guard<std::mutex> lock(g_pool_mutex);
+    QueuePool& P = g_pools[l.dev];
+    if (cudaEventRecord(P.done[l.slot], stream) != cudaSuccess) {
+        cudaGetLastError();
+        cudaStreamSynchronize(stream);  // cannot track it: wait, then the slot is free
+        P.used[l.slot] = false;
+    }
+    P.pending[l.slot] = false;
 }
 
 int fail(int rc, const char* fmt, ...) {
@@ -179,13 +232,18 @@ int run_common(int what, const chs_problem* pb, long long n_ic, double* y, doubl
         a.n_rej = rep->n_rejected;
         a.status = rep->status;
         a.t_final = rep->t_final;
+        a.carry = rep->carry;
+        a.resume = rep->resume ? 1 : 0;
     }
     if (n_ic == 0 && !info) return CHS_OK;
+    QueueLease lease;
     if (st->adaptive && !info && g_adaptive_refill.load() != 0 && pb->system != CHS_SYS_DOUBLE_PENDULUM) {
-        a.queue = acquire_queue(rq.stream);
-        if (!a.queue) return fail(CHS_ECUDA, "could not set up the lane-refill work queue");
+        lease = acquire_queue(rq.stream);
+        a.queue = lease.counter;  // nullptr (every counter busy): launch without refill, same results
     }
-    return finish(dispatch(rq), rq);
+    const int r = dispatch(rq);
+    release_after_launch(lease, rq.stream);
+    return finish(r, rq);
 }
 
 }  // namespace
@@ -321,22 +379,54 @@ int chaoticus_kernel_info(const chs_problem* pb, int what, int k, int adaptive, 
 
 // ---- host-buffer forms ---------------------------------------------------------------------
 namespace {
+// Scratch of the host-buffer entry points: one internal stream per host thread, created on first use
+// and kept; device buffers come from the stream-ordered allocator (cudaMallocAsync) whose pool keeps
+// freed memory (release threshold = unlimited), so after the first call an allocation is a pool
+// look-up, not a cudaMalloc.
+struct HostCtx {
+    cudaStream_t stream = nullptr;
+    int dev = -1;
+};
+thread_local HostCtx g_host;
+
+cudaError_t host_stream(cudaStream_t* out) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (!g_host.stream || g_host.dev != dev) {
+        if (g_host.stream) cudaStreamDestroy(g_host.stream);
+        g_host.stream = nullptr;
+        e = cudaStreamCreateWithFlags(&g_host.stream, cudaStreamNonBlocking);
+        if (e != cudaSuccess) return e;
+        g_host.dev = dev;
+        cudaMemPool_t pool;
+        if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+            unsigned long long keep = ~0ULL;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        }
+    }
+    *out = g_host.stream;
+    return cudaSuccess;
+}
+
 struct DevBuf {
     void* p = nullptr;
     size_t bytes = 0;
+    cudaStream_t st = nullptr;
     ~DevBuf() {
-        if (p) cudaFree(p);
+        if (p) cudaFreeAsync(p, st);
     }
-    cudaError_t alloc(size_t b) {
+    cudaError_t alloc(size_t b, cudaStream_t stream) {
         bytes = b;
-        return b ? cudaMalloc(&p, b) : cudaSuccess;
+        st = stream;
+        return b ? cudaMallocAsync(&p, b, stream) : cudaSuccess;
     }
 };
 #define CK(x)                                                                                  \
     do {                                                                                       \
         cudaError_t e_ = (x);                                                                  \
         if (e_ != cudaSuccess) {                                                               \
-            if (stream) cudaStreamDestroy(stream);                                             \
+            if (stream) cudaStreamSynchronize(stream);                                         \
             return fail(CHS_ECUDA, "CUDA error %d: %s", (int)e_, cudaGetErrorString(e_));      \
         }                                                                                      \
     } while (0)
@@ -355,27 +445,30 @@ int run_host(int what, const chs_problem* pb, long long n_ic, double* y, double*
     const long long ns = st->adaptive ? 1 : chaoticus_n_samples(st->n_steps, renorm_every, sample_every);
     const size_t by = sizeof(double) * (size_t)n * n_ic, bw = by * (size_t)k, bs = sizeof(double) * (size_t)ns * n_ic,
                  bk = sizeof(double) * (size_t)k * n_ic;
-    DevBuf dy, dw, ds, dl, dlam, dacc, drej, dstat, dtf;
-    CK(cudaStreamCreate(&stream));
-    CK(dy.alloc(by));
-    CK(dw.alloc(bw));
-    if (series) CK(ds.alloc(bs));
-    if (logacc) CK(dl.alloc(bk));
-    if (lambda) CK(dlam.alloc(bk));
-    chs_report drep{nullptr, nullptr, nullptr, nullptr};
+    DevBuf dy, dw, ds, dl, dlam, dacc, drej, dstat, dtf, dcar;
+    CK(host_stream(&stream));
+    CK(dy.alloc(by, stream));
+    CK(dw.alloc(bw, stream));
+    if (series) CK(ds.alloc(bs, stream));
+    if (logacc) CK(dl.alloc(bk, stream));
+    if (lambda) CK(dlam.alloc(bk, stream));
+    chs_report drep{nullptr, nullptr, nullptr, nullptr, nullptr, 0};
     if (rep) {
-        if (rep->n_accepted) { CK(dacc.alloc(sizeof(long long) * n_ic)); drep.n_accepted = (long long*)dacc.p; }
-        if (rep->n_rejected) { CK(drej.alloc(sizeof(long long) * n_ic)); drep.n_rejected = (long long*)drej.p; }
-        if (rep->status) { CK(dstat.alloc(sizeof(int) * n_ic)); drep.status = (int*)dstat.p; }
-        if (rep->t_final) { CK(dtf.alloc(sizeof(double) * n_ic)); drep.t_final = (double*)dtf.p; }
+        drep.resume = rep->resume;
+        if (rep->carry) { CK(dcar.alloc(by, stream)); drep.carry = (double*)dcar.p; }
+        if (rep->n_accepted) { CK(dacc.alloc(sizeof(long long) * n_ic, stream)); drep.n_accepted = (long long*)dacc.p; }
+        if (rep->n_rejected) { CK(drej.alloc(sizeof(long long) * n_ic, stream)); drep.n_rejected = (long long*)drej.p; }
+        if (rep->status) { CK(dstat.alloc(sizeof(int) * n_ic, stream)); drep.status = (int*)dstat.p; }
+        if (rep->t_final) { CK(dtf.alloc(sizeof(double) * n_ic, stream)); drep.t_final = (double*)dtf.p; }
     }
     CK(cudaMemcpyAsync(dy.p, y, by, cudaMemcpyHostToDevice, stream));
     if (k > 0) CK(cudaMemcpyAsync(dw.p, w, bw, cudaMemcpyHostToDevice, stream));
     if (logacc) CK(cudaMemcpyAsync(dl.p, logacc, bk, cudaMemcpyHostToDevice, stream));
+    if (drep.carry && drep.resume) CK(cudaMemcpyAsync(dcar.p, rep->carry, by, cudaMemcpyHostToDevice, stream));
     rc = run_common(what, pb, n_ic, (double*)dy.p, (double*)dw.p, k, st, renorm_every, sample_every, (double*)ds.p,
                     (double*)dl.p, (double*)dlam.p, &drep, stream, nullptr);
     if (rc) {
-        cudaStreamDestroy(stream);
+        cudaStreamSynchronize(stream);
         return rc;
     }
     CK(cudaMemcpyAsync(y, dy.p, by, cudaMemcpyDeviceToHost, stream));
@@ -388,9 +481,9 @@ int run_host(int what, const chs_problem* pb, long long n_ic, double* y, double*
         if (rep->n_rejected) CK(cudaMemcpyAsync(rep->n_rejected, drej.p, sizeof(long long) * n_ic, cudaMemcpyDeviceToHost, stream));
         if (rep->status) CK(cudaMemcpyAsync(rep->status, dstat.p, sizeof(int) * n_ic, cudaMemcpyDeviceToHost, stream));
         if (rep->t_final) CK(cudaMemcpyAsync(rep->t_final, dtf.p, sizeof(double) * n_ic, cudaMemcpyDeviceToHost, stream));
+        if (rep->carry) CK(cudaMemcpyAsync(rep->carry, dcar.p, by, cudaMemcpyDeviceToHost, stream));
     }
     CK(cudaStreamSynchronize(stream));
-    cudaStreamDestroy(stream);
     return CHS_OK;
 }
 }  // namespace
@@ -405,20 +498,19 @@ int chaoticus_ld_host(const chs_problem* pb, long long n_ic, const double* y0, d
     if (!y0) return fail(CHS_EINVAL, "y0 is NULL");
     DevBuf dy, df, db;
     const size_t by = sizeof(double) * (size_t)n * n_ic, bo = sizeof(double) * (size_t)n_ic;
-    CK(cudaStreamCreate(&stream));
-    CK(dy.alloc(by));
-    if (ld_fwd) CK(df.alloc(bo));
-    if (ld_bwd) CK(db.alloc(bo));
+    CK(host_stream(&stream));
+    CK(dy.alloc(by, stream));
+    if (ld_fwd) CK(df.alloc(bo, stream));
+    if (ld_bwd) CK(db.alloc(bo, stream));
     CK(cudaMemcpyAsync(dy.p, y0, by, cudaMemcpyHostToDevice, stream));
     int rc = chaoticus_ld(pb, n_ic, (const double*)dy.p, t0, h, n_steps, (double*)df.p, (double*)db.p, stream);
     if (rc) {
-        cudaStreamDestroy(stream);
+        cudaStreamSynchronize(stream);
         return rc;
     }
     if (ld_fwd) CK(cudaMemcpyAsync(ld_fwd, df.p, bo, cudaMemcpyDeviceToHost, stream));
     if (ld_bwd) CK(cudaMemcpyAsync(ld_bwd, db.p, bo, cudaMemcpyDeviceToHost, stream));
     CK(cudaStreamSynchronize(stream));
-    cudaStreamDestroy(stream);
     return CHS_OK;
 }
 

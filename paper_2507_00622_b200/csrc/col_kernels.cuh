@@ -48,6 +48,9 @@ struct RunArgs {
     long long* n_rej;
     int* status;
     double* t_final;
+    // continuation (include/chaoticus.h chs_report): carried rounding words of the orbit, [n][n_ic]
+    double* carry;
+    int resume;
     // Lagrangian descriptor
     const double* y0;
     double* ld_fwd;
@@ -176,6 +179,41 @@ struct Col {
         }
     }
 
+    // carried rounding words of the orbit's compensated update (items 0..ND-1 of the orbit lane)
+    // across a call boundary: carry[c][ic] in the layout of y
+    __device__ __forceinline__ void load_carry(const double* cw, long long n_ic, long long ic, double (&qc)[ND],
+                                               double (&pc)[ND]) const {
+        if (lt == 0) {
+#pragma unroll
+            for (int d = 0; d < ND; d++) {
+                qc[d] = cw[(long long)d * n_ic + ic];
+                pc[d] = cw[(long long)(ND + d) * n_ic + ic];
+            }
+        }
+    }
+    __device__ __forceinline__ void store_carry(double* cw, long long n_ic, long long ic, const double (&qc)[ND],
+                                                const double (&pc)[ND], bool bad) const {
+        if (lt == 0) {
+#pragma unroll
+            for (int d = 0; d < ND; d++) {
+                cw[(long long)d * n_ic + ic] = bad ? 0.0 : qc[d];
+                cw[(long long)(ND + d) * n_ic + ic] = bad ? 0.0 : pc[d];
+            }
+        }
+    }
+    // On the other lanes of a multi-lane tile item 0 is a deviation column; the step code is the
+    // same for every lane, so that column carries a rounding word too.  It is dropped at every
+    // renormalisation (the vector is rescaled there anyway), so that no deviation word ever has
+    // to cross a call boundary.
+    __device__ __forceinline__ void scrub_carry(double (&qc)[ND], double (&pc)[ND]) const {
+        if constexpr (L > 1) {
+            if (lt != 0) {
+#pragma unroll
+                for (int d = 0; d < ND; d++) qc[d] = pc[d] = 0.0;
+            }
+        }
+    }
+
     // force on all items at stage coordinates Q (Eq.(5) etc. + variational part)
     __device__ __forceinline__ void force(const double (&Q)[NI], double (&F)[NI]) const {
         double Qo[ND];
@@ -264,7 +302,7 @@ struct Col {
 #pragma unroll
             for (int j = 0; j < CPL; j++) {
                 const int c = col_of(j);
-                if ((L == 1) ? (j > v) : (c > v && c < NCOL && apply)) {
+                if ((L == 1) ? (j > v && apply) : (c > v && c < NCOL && apply)) {
                     double dot = 0.0;
 #pragma unroll
                     for (int d = 0; d < ND; d++) dot = fma(wq[d], q[j * ND + d], dot);
@@ -337,7 +375,7 @@ struct Col {
                     const long long o = (long long)(col_of(j) - 1) * a.n_ic + ic;
                     const double lv = logacc_value(lg[j]);
                     if (a.logacc) a.logacc[o] = bad ? nan("") : a.logacc[o] + lv;
-                    if (a.lambda) a.lambda[o] = (bad || elapsed == 0.0) ? nan("") : lv / elapsed;
+                    if (a.lambda) a.lambda[o] = (bad || elapsed == 0.0) ? nan("") : lv / fabs(elapsed);
                 }
             }
         }
@@ -448,7 +486,11 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
         const bool valid = traj < a.n_ic;
         const long long ic = valid ? traj : a.n_ic - 1;  // padding tiles shadow the last trajectory
         s.load(a.y, a.w, a.n_ic, ic, 1.0);
-        s.template do_renorm<MODE>(false, true);  // on entry: no log accumulated
+        if (a.resume) {
+            if (a.carry) s.load_carry(a.carry, a.n_ic, ic, qc, pc);
+        } else {
+            s.template do_renorm<MODE>(false, true);  // on entry: no log accumulated
+        }
         long long slot = 0;
         int cd = a.m, sd = a.sample_every;
         for (long long st = 1; st <= a.n_steps; ++st) {
@@ -470,6 +512,7 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
                 if (--cd == 0 || st == a.n_steps) {
                     cd = a.m;
                     s.template do_renorm<MODE>(want_log, true);
+                    s.scrub_carry(qc, pc);
                     if constexpr (IND != IND_NONE) {
                         if (a.sample_every > 0 && --sd == 0) {
                             sd = a.sample_every;
@@ -491,6 +534,7 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
         if constexpr (IND != IND_NONE) ind = s.template indicator<IND>();
         if (!valid) return;
         s.store(a.y, a.w, a.n_ic, ic, bad);
+        if (a.carry) s.store_carry(a.carry, a.n_ic, ic, qc, pc, bad);
         if constexpr (K > 0) s.store_logs(a, ic, bad, t - a.t0);
         if (s.lt == 0) {
             if constexpr (IND != IND_NONE) {
@@ -544,7 +588,7 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
 #pragma unroll
                     for (int c = 0; c < NC; c++) qc[c] = pc[c] = 0.0;
                 }
-                s.template do_renorm<MODE>(false, got);  // on entry: no log accumulated
+                s.template do_renorm<MODE>(false, got && !a.resume);  // on entry: no log accumulated
                 const double h_init = a.h0 > 0.0 ? a.h0 : initial_step(s, interval, dir, a.rtol, a.atol);
                 if (got) h_abs = h_init;
                 need = false;
@@ -614,7 +658,10 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
                 }
             }
             if constexpr (MODE != MODE_NONE) {
-                if (__any_sync(0xffffffffu, ren)) s.template do_renorm<MODE>(want_log, ren);
+                if (__any_sync(0xffffffffu, ren)) {
+                    s.template do_renorm<MODE>(want_log, ren);
+                    if (ren) s.scrub_carry(qc, pc);
+                }
             }
 
             // trajectories that ended in this iteration: write their results, ask for the next one

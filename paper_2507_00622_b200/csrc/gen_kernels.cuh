@@ -85,7 +85,7 @@ gen_run_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, 
 #pragma unroll
     for (int c = 0; c < N; c++) {
         y[c] = a.y[(long long)c * a.n_ic + ic];
-        yc[c] = 0.0;
+        yc[c] = (a.resume && a.carry) ? a.carry[(long long)c * a.n_ic + ic] : 0.0;
     }
     long long n_acc = 0, n_rej = 0;
     int status = ST_OK;
@@ -226,6 +226,10 @@ gen_run_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, 
     if (bad && status == ST_OK) status = ST_NONFINITE;
 #pragma unroll
     for (int c = 0; c < N; c++) a.y[(long long)c * a.n_ic + ic] = bad ? nan("") : y[c];
+    if (a.carry) {
+#pragma unroll
+        for (int c = 0; c < N; c++) a.carry[(long long)c * a.n_ic + ic] = bad ? 0.0 : yc[c];
+    }
     if (a.n_acc) a.n_acc[ic] = n_acc;
     if (a.n_rej) a.n_rej[ic] = n_rej;
     if (a.status) a.status[ic] = status;

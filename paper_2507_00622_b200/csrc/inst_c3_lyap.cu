@@ -1,5 +1,6 @@
-// inst_c3_lyap.cu -- 3-DoF coupled oscillators: full Lyapunov spectrum (BASELINE configs[3]):
-// 8-lane tile per trajectory, lane v holds column v (orbit, w1..w6), lane 7 idle.
+// inst_c3_lyap.cu -- 3-DoF coupled oscillators: full Lyapunov spectrum (BASELINE configs[3]).
+// Fixed step: 4-lane tile per trajectory, two columns per lane (orbit + w1 | w2, w3 | w4, w5 | w6 and one
+// empty slot).  Adaptive: 8-lane tile, one column per lane (lane 7 idle).  Also GALI_2, GALI_3.
 #include "launch.h"
 namespace chs {
 int try_launch_c3_lyap(const LaunchReq& rq) {

@@ -118,6 +118,55 @@ def test_hh_adaptive_gali_lyap(chs, orc, k):
     assert lam_err(lg, lo, 40.0) <= 1e-6
 
 
+@pytest.mark.parametrize("k", [1, 2])
+def test_hh_adaptive_lyap_thread_layout(chs, orc, k):
+    """Adaptive Lyapunov k = 1, 2 on the ONE-THREAD-PER-TRAJECTORY layout, on an unequal ensemble
+    (E = 1/6 orbits interleaved with E = 0.01 orbits): a lane's Gram-Schmidt projection must only
+    act when that lane renormalises, not whenever a warp-mate does (predicate `apply` of Col::mgs)
+    -- against the oracle, and bit-identical with lane refill on and off."""
+    import torch
+    ya, yb = W.hh_grid(1.0 / 6.0, 20, 10), W.hh_grid(0.01, 20, 10)
+    y0 = np.empty((4, 400))
+    y0[:, 0::2], y0[:, 1::2] = ya, yb
+    w0 = W.deviation_vectors(400, k, 4, 33, "raw")
+    assert chs.kernel_info(HH, None, chs.WHAT_LYAP, k=k, adaptive=True, n_ic=400)["lanes"] == 1
+    st = dict(adaptive=True, t_end=60.0, rtol=1e-11, atol=1e-11)
+    yo, wo = y0.copy(), w0.copy()
+    lo = orc.lyap(HH, None, yo, wo, renorm_every=3, precision="f80", **st)["lam"]
+    outs = {}
+    try:
+        for mode in (0, 1):
+            chs.set_option("adaptive_refill", mode)
+            yg, wg, rep = dev(y0), dev(w0), chs.Report(400, "cuda")
+            lg = chs.lyap(HH, None, yg, wg, renorm_every=3, report=rep, **st)
+            outs[mode] = [t.clone() for t in (lg, yg, wg, rep.n_accepted, rep.n_rejected)]
+    finally:
+        chs.set_option("adaptive_refill", 1)
+    for a, b in zip(outs[0], outs[1]):
+        assert torch.equal(a, b)
+    lg, yg, wg = (t.cpu().numpy() for t in outs[1][:3])
+    acc = outs[1][3].cpu().numpy()
+    assert acc.max() > 1.3 * acc.min()
+    assert lam_err(lg, lo, 60.0) <= 1e-6
+    assert rel_state(yg, yo).max() <= 1e-8 and np.abs(wg - wo).max() <= 1e-6
+
+
+def test_lyap_backward_time(chs, orc):
+    """Backward-time runs (h < 0, or t_end < t0): exponents are growth rates per unit of |t|
+    (R18), so a chaotic orbit's largest exponent is positive in both time directions."""
+    cfg = W.config("C3", n_ic=100)
+    y0 = cfg["y"]
+    w0 = W.deviation_vectors(100, 2, 4, 5, "orthonormal")
+    lo = orc.lyap(HH, None, y0.copy(), w0.copy(), renorm_every=5, h=-0.02, n_steps=4000, precision="f80")["lam"]
+    lg = chs.lyap(HH, None, dev(y0), dev(w0), renorm_every=5, h=-0.02, n_steps=4000).cpu().numpy()
+    assert lam_err(lg, lo, 80.0) <= 1e-8
+    assert lg[0].max() > 0.02 and (lg[0] > -1e-3).all()
+    st = dict(adaptive=True, t_end=-40.0, rtol=1e-11, atol=1e-11)
+    lo = orc.lyap(HH, None, y0.copy(), w0.copy(), renorm_every=2, precision="f80", **st)["lam"]
+    lg = chs.lyap(HH, None, dev(y0), dev(w0), renorm_every=2, **st).cpu().numpy()
+    assert lam_err(lg, lo, 40.0) <= 1e-6 and (lg[0] > -1e-3).all()
+
+
 @pytest.mark.parametrize("k", [2, 3, 4, 5])
 def test_coupled3_lyap_other_k(chs, orc, k):
     cfg = W.config("C4", n_ic=77)

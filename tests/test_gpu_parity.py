@@ -81,16 +81,25 @@ def test_integrate_fixed_coupled3(chs, orc):
 
 
 def test_resume(chs):
-    """In-place continuation (checkpoint / resume): one call of n steps == two calls of n/2, up to
-    the carried rounding word of the compensated orbit update, which a call boundary drops
-    (<= 1 ulp per boundary)."""
+    """In-place continuation (checkpoint / resume): with the carried rounding
+    words of the compensated orbit update handed over (chs_report.carry, resume = 1) one call of n
+    steps == two calls, BIT FOR BIT.  Without the carry the boundary drops one rounding word per
+    component (<= 1 ulp)."""
     y0 = W.hh_grid(0.125, 16, 16)
     a = dev(y0)
     b = dev(y0)
     chs.integrate_fixed(HH, None, a, 0.0, 0.01, 1000)
-    chs.integrate_fixed(HH, None, b, 0.0, 0.01, 400)
-    chs.integrate_fixed(HH, None, b, 4.0, 0.01, 600)
-    assert rel_state(b.cpu().numpy(), a.cpu().numpy()).max() <= 1e-13
+    rep = chs.Report(256, "cuda", n=4)
+    chs.integrate_fixed(HH, None, b, 0.0, 0.01, 400, report=rep)
+    assert rep.carry.abs().max().item() > 0.0
+    rep.resume = True
+    chs.integrate_fixed(HH, None, b, 4.0, 0.01, 600, report=rep)
+    assert (a == b).all().item()
+    # without the carry: last-digit differences only
+    d = dev(y0)
+    chs.integrate_fixed(HH, None, d, 0.0, 0.01, 400)
+    chs.integrate_fixed(HH, None, d, 4.0, 0.01, 600)
+    assert rel_state(d.cpu().numpy(), a.cpu().numpy()).max() <= 1e-13
     # and a repeated call is deterministic, bit for bit
     c = dev(y0)
     chs.integrate_fixed(HH, None, c, 0.0, 0.01, 1000)
@@ -238,17 +247,70 @@ def test_sali_renorm_interval_and_tail(chs, orc):
     assert np.abs(wg.cpu().numpy() - wo).max() <= 1e-10
 
 
-def test_sali_resume(chs):
-    y0, w0 = _sali_case(12)
+@pytest.mark.parametrize("n_side", [12, 70])   # 4-lane tile (<= 4096 ICs) and one thread per trajectory
+def test_sali_resume(chs, n_side):
+    """Split at a multiple of renorm_every with carry + resume: y, w and SALI bit-identical."""
+    y0, w0 = _sali_case(n_side)
+    n_ic = y0.shape[1]
     a_y, a_w = dev(y0), dev(w0)
     b_y, b_w = dev(y0), dev(w0)
     sa = chs.sali(HH, None, a_y, a_w, renorm_every=5, h=0.01, n_steps=1000)
-    chs.sali(HH, None, b_y, b_w, renorm_every=5, h=0.01, n_steps=500)
-    sb = chs.sali(HH, None, b_y, b_w, renorm_every=5, t0=5.0, h=0.01, n_steps=500)
-    # a call boundary drops the orbit's carried rounding word and re-normalises the already-unit
-    # vectors (|w| = 1 +- ulp): last-digit differences only
-    assert rel_state(b_y.cpu().numpy(), a_y.cpu().numpy()).max() <= 1e-13
-    assert (a_w - b_w).abs().max().item() <= 1e-12 and ((sa - sb).abs() / sa).max().item() <= 1e-11
+    rep = chs.Report(n_ic, "cuda", n=4)
+    chs.sali(HH, None, b_y, b_w, renorm_every=5, h=0.01, n_steps=500, report=rep)
+    rep.resume = True
+    sb = chs.sali(HH, None, b_y, b_w, renorm_every=5, t0=5.0, h=0.01, n_steps=500, report=rep)
+    assert (a_y == b_y).all().item() and (a_w == b_w).all().item() and (sa == sb).all().item()
+    # without carry / resume: the boundary drops the orbit's carried word and re-normalises the
+    # already-unit vectors (|w| = 1 +- ulp): last-digit differences only
+    c_y, c_w = dev(y0), dev(w0)
+    chs.sali(HH, None, c_y, c_w, renorm_every=5, h=0.01, n_steps=500)
+    sc = chs.sali(HH, None, c_y, c_w, renorm_every=5, t0=5.0, h=0.01, n_steps=500)
+    assert rel_state(c_y.cpu().numpy(), a_y.cpu().numpy()).max() <= 1e-13
+    assert (a_w - c_w).abs().max().item() <= 1e-12 and ((sa - sc).abs() / sa).max().item() <= 1e-11
+
+
+def test_resume_all_layouts(chs):
+    """Bit-identical continuation on every layout: column tile with two columns per lane + MGS (C4's
+    kernel), chain tile + GALI (C5's kernel), one thread per trajectory + MGS, the generic kernel."""
+    import torch
+    cases = []
+    cfg = W.config("C4", n_ic=203)
+    cases.append(("lyap", C3, cfg["params"], cfg["y"], cfg["w"], 0.01, 6))
+    cfg = W.config("C5", n_ic=101)
+    cases.append(("gali", FPUT, cfg["params"], cfg["y"], cfg["w"], 0.05, 16))
+    y0 = W.hh_grid(0.125, 11, 13)
+    cases.append(("lyap", HH, None, y0, W.deviation_vectors(143, 2, 4, 12, "orthonormal"), 0.01, 4))
+    for what, sysid, prm, y0, w0, h, n in cases:
+        fn = getattr(chs, what)
+        n_ic = y0.shape[1]
+        a_y, a_w, b_y, b_w = dev(y0), dev(w0), dev(y0), dev(w0)
+        oa = fn(sysid, prm, a_y, a_w, renorm_every=10, h=h, n_steps=600)
+        rep = chs.Report(n_ic, "cuda", n=n)
+        fn(sysid, prm, b_y, b_w, renorm_every=10, h=h, n_steps=250, report=rep)
+        rep.resume = True
+        ob = fn(sysid, prm, b_y, b_w, renorm_every=10, t0=250 * h, h=h, n_steps=350, report=rep)
+        assert torch.equal(a_y, b_y) and torch.equal(a_w, b_w), (what, sysid)
+        if what == "gali":
+            assert torch.equal(oa, ob)
+    DP = W.SYS_DOUBLE_PENDULUM
+    y0 = W.double_pendulum_ics(200, seed=3)
+    a, b = dev(y0), dev(y0)
+    chs.integrate_fixed(DP, (1.0, 1.0), a, 0.0, 0.01, 500)
+    rep = chs.Report(200, "cuda", n=4)
+    chs.integrate_fixed(DP, (1.0, 1.0), b, 0.0, 0.01, 123, report=rep)
+    rep.resume = True
+    chs.integrate_fixed(DP, (1.0, 1.0), b, 1.23, 0.01, 377, report=rep)
+    assert torch.equal(a, b)
+    # host-buffer entry point: the carry travels through host memory
+    y0, w0 = _sali_case(9)
+    yh, wh, sh = y0.copy(), w0.copy(), np.empty((1, 81))
+    hrep = chs.HostReport(81, n=4)
+    chs.sali_host(HH, None, yh, wh, sh, renorm_every=1, h=0.01, n_steps=100, report=hrep)
+    hrep.resume = True
+    chs.sali_host(HH, None, yh, wh, sh, renorm_every=1, t0=1.0, h=0.01, n_steps=200, report=hrep)
+    yg, wg = dev(y0), dev(w0)
+    sg = chs.sali(HH, None, yg, wg, renorm_every=1, h=0.01, n_steps=300)
+    assert (sg.cpu().numpy() == sh).all() and (yg.cpu().numpy() == yh).all() and (wg.cpu().numpy() == wh).all()
 
 
 def test_sali_host_entry(chs):
