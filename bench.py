@@ -58,6 +58,7 @@ def parse():
     ap.add_argument("--fput-n", type=int, default=8, help="F3: chain length (4, 8, 16, 32)")
     ap.add_argument("--n-ic", type=int, default=1000, help="F3: ensemble size (PAPER.md:129: 10^3 random ICs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--tune", type=int, default=0, help="development: kernel variant knob (chaoticus_set_option)")
     return ap.parse_args()
 
 
@@ -309,6 +310,8 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    if args.tune:
+        chs.set_option("tune", args.tune)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
     wk = make_workload(chs, torch, args, rank, world)
     wl, step_dev, step_e2e, h2d, d2h, kinfo = wk["wl"], wk["step_dev"], wk["step_e2e"], wk["h2d"], wk["d2h"], wk["kinfo"]

@@ -1,61 +1,85 @@
 // chain_kernels.cuh -- "chain layout" for the FPUT chain (CUDA path, sm_100a).
 //
 // PAPER.md:98-111 Eq.(6)-(8): N particles, fixed ends, nearest-neighbour springs.  A trajectory
-// is owned by a tile of L = N lanes (N = 2, 4, 8, 16, 32; one full warp per trajectory at
-// N = 32), lane i <-> particle i+1.  A lane holds, for its particle, the orbit coordinate and
-// the K deviation-vector coordinates: 1 + K (q, p) pairs and their stage forces, all in
-// registers.  Neighbour coupling goes through warp shuffles: per column one shuffle up (the left
-// neighbour's stage coordinate) and one shuffle down (the right spring's force, computed by the
-// right neighbour), so every spring is evaluated once.  Norms, dot products, Gram-Schmidt and
-// the Jacobi rotations of GALI_k's SVD are butterfly shuffle reductions over the tile
-// (BASELINE.json north_star, configs[4]).
+// is owned by a tile of LT consecutive lanes (LT = 2..32, a power of two), each lane holding PPL
+// consecutive particles: lane l <-> particles l PPL + 1 .. (l + 1) PPL.  For each of its particles a
+// lane holds the orbit coordinate and the K deviation-vector coordinates: PPL (1 + K) (q, p) pairs
+// and their stage forces, all in registers.
+//   * Neighbour coupling goes through warp shuffles of the STAGE COORDINATES only: per column one
+//     shuffle up (the left neighbour's last particle) and one shuffle down (the right neighbour's
+//     first particle), both issued before any arithmetic; springs between two particles of the same
+//     lane need none.  A lane evaluates the PPL + 1 springs that touch its particles (the spring it
+//     shares with its right neighbour is evaluated by both: one redundant spring per lane instead of
+//     a second, dependent shuffle).  The walls q_0 = q_{N+1} = 0 (Eq.(8)) are the zeros the first /
+//     last lane substitutes for the missing neighbour, so there is no wall branch.
+//   * PPL = 2 halves the shuffles per particle and removes a third of the spring arithmetic
+//     (BASELINE.json configs[4] runs as LT = 4, PPL = 2: DESIGN.md "Layouts").
+//   * PAD: chains whose length is not LT PPL are padded with particles pinned at zero (coordinates
+//     start at 0 and their force is masked to 0), which act as the right wall; np is the real length.
+//   * Norms, dot products, Gram-Schmidt and the Jacobi rotations of GALI_k's SVD are lane-local sums
+//     followed by butterfly shuffle reductions over the tile (bit-identical on all lanes).
 #pragma once
 #include "col_kernels.cuh"
 
 namespace chs {
 
-template <int NP, int K_>
+template <int LT, int PPL_, int K_, bool PAD_ = false, bool COLD_ = false>
 struct Chain {
-    static constexpr int K = K_, L = NP;
+    static constexpr int K = K_, L = LT, PPL = PPL_;
+    static constexpr bool PAD = PAD_;
+    static constexpr bool COLD = COLD_;  // carry words and log accumulators in shared memory
     static constexpr int NCOL = 1 + K;
-    static constexpr int NI = NCOL;
-    static constexpr int N = 2 * NP;
-    static constexpr int D = N * NCOL;
-    static constexpr int NCOMP = 1;  // item 0: the orbit coordinate -- compensated update
+    static constexpr int NI = NCOL * PPL;  // item v * PPL + j: column v (0 = orbit), local particle j
+    static constexpr int NSLOT = LT * PPL;
+    static constexpr int NCOMP = PPL;      // items 0..PPL-1: the orbit coordinates -- compensated update
     using Params = FputParams;
 
     Params prm;
     int lt;
+    int np;   // real chain length (== NSLOT unless PAD)
+    mutable int par;  // wide tiles: which half of the edge buffer the next exchange uses
     double q[NI], p[NI];
-    LogAcc lg[NCOL];  // deferred-log accumulators, lg[v], v >= 1: identical on all lanes of the tile
+    LogBank<NCOL, COLD> lg;  // deferred-log accumulators, v >= 1: identical on all lanes of the tile
 
     __device__ __forceinline__ void init(const Params& P) {
         prm = P;
         lt = (int)(threadIdx.x % L);
-#pragma unroll
-        for (int j = 0; j < NCOL; j++) logacc_init(lg[j]);
+        np = PAD ? P.np : NSLOT;
+        par = 0;
+        lg.init();
     }
-    __device__ __forceinline__ void reset_logs() {
-#pragma unroll
-        for (int j = 0; j < NCOL; j++) logacc_init(lg[j]);
-    }
+    __device__ __forceinline__ double dcount() const { return (double)(2 * np * NCOL); }
+    __device__ __forceinline__ bool real(int j) const { return !PAD || lt * PPL + j < np; }
+    __device__ __forceinline__ void reset_logs() { lg.init(); }
     __device__ __forceinline__ void load(const double* y, const double* w, long long n_ic, long long ic,
                                          double psign) {
-        q[0] = y[(long long)lt * n_ic + ic];
-        p[0] = psign * y[(long long)(NP + lt) * n_ic + ic];
+        const int n = 2 * np;
 #pragma unroll
-        for (int v = 1; v < NCOL; v++) {
-            q[v] = w[((long long)(v - 1) * N + lt) * n_ic + ic];
-            p[v] = w[((long long)(v - 1) * N + NP + lt) * n_ic + ic];
+        for (int j = 0; j < PPL; j++) {
+            const int pi = lt * PPL + j;
+            const bool on = real(j);
+            q[j] = on ? y[(long long)pi * n_ic + ic] : 0.0;
+            p[j] = on ? psign * y[(long long)(np + pi) * n_ic + ic] : 0.0;
+#pragma unroll
+            for (int v = 1; v < NCOL; v++) {
+                q[v * PPL + j] = on ? w[((long long)(v - 1) * n + pi) * n_ic + ic] : 0.0;
+                p[v * PPL + j] = on ? w[((long long)(v - 1) * n + np + pi) * n_ic + ic] : 0.0;
+            }
         }
     }
     __device__ __forceinline__ void store(double* y, double* w, long long n_ic, long long ic, bool bad) const {
-        y[(long long)lt * n_ic + ic] = bad ? nan("") : q[0];
-        y[(long long)(NP + lt) * n_ic + ic] = bad ? nan("") : p[0];
+        const int n = 2 * np;
 #pragma unroll
-        for (int v = 1; v < NCOL; v++) {
-            w[((long long)(v - 1) * N + lt) * n_ic + ic] = bad ? nan("") : q[v];
-            w[((long long)(v - 1) * N + NP + lt) * n_ic + ic] = bad ? nan("") : p[v];
+        for (int j = 0; j < PPL; j++) {
+            const int pi = lt * PPL + j;
+            if (!real(j)) continue;
+            y[(long long)pi * n_ic + ic] = bad ? nan("") : q[j];
+            y[(long long)(np + pi) * n_ic + ic] = bad ? nan("") : p[j];
+#pragma unroll
+            for (int v = 1; v < NCOL; v++) {
+                w[((long long)(v - 1) * n + pi) * n_ic + ic] = bad ? nan("") : q[v * PPL + j];
+                w[((long long)(v - 1) * n + np + pi) * n_ic + ic] = bad ? nan("") : p[v * PPL + j];
+            }
         }
     }
     __device__ __forceinline__ void store_logs(const RunArgs& a, long long ic, bool bad, double elapsed) const {
@@ -63,59 +87,124 @@ struct Chain {
 #pragma unroll
         for (int v = 1; v < NCOL; v++) {
             const long long o = (long long)(v - 1) * a.n_ic + ic;
-            const double lv = logacc_value(lg[v]);
+            const double lv = lg.value(v);
             if (a.logacc) a.logacc[o] = bad ? nan("") : a.logacc[o] + lv;
             if (a.lambda) a.lambda[o] = (bad || elapsed == 0.0) ? nan("") : lv / fabs(elapsed);
         }
     }
-    // carried rounding word of this particle's orbit coordinate across a call boundary
-    __device__ __forceinline__ void load_carry(const double* cw, long long n_ic, long long ic, double (&qc)[1],
-                                               double (&pc)[1]) const {
-        qc[0] = cw[(long long)lt * n_ic + ic];
-        pc[0] = cw[(long long)(NP + lt) * n_ic + ic];
+    // carried rounding words of this lane's orbit coordinates across a call boundary
+    __device__ __forceinline__ void load_carry(const double* cw, long long n_ic, long long ic, double (&qc)[PPL],
+                                               double (&pc)[PPL]) const {
+#pragma unroll
+        for (int j = 0; j < PPL; j++) {
+            const int pi = lt * PPL + j;
+            qc[j] = real(j) ? cw[(long long)pi * n_ic + ic] : 0.0;
+            pc[j] = real(j) ? cw[(long long)(np + pi) * n_ic + ic] : 0.0;
+        }
     }
-    __device__ __forceinline__ void store_carry(double* cw, long long n_ic, long long ic, const double (&qc)[1],
-                                                const double (&pc)[1], bool bad) const {
-        cw[(long long)lt * n_ic + ic] = bad ? 0.0 : qc[0];
-        cw[(long long)(NP + lt) * n_ic + ic] = bad ? 0.0 : pc[0];
+    __device__ __forceinline__ void store_carry(double* cw, long long n_ic, long long ic, const double (&qc)[PPL],
+                                                const double (&pc)[PPL], bool bad) const {
+#pragma unroll
+        for (int j = 0; j < PPL; j++) {
+            const int pi = lt * PPL + j;
+            if (!real(j)) continue;
+            cw[(long long)pi * n_ic + ic] = bad ? 0.0 : qc[j];
+            cw[(long long)(np + pi) * n_ic + ic] = bad ? 0.0 : pc[j];
+        }
     }
-    __device__ __forceinline__ void scrub_carry(double (&)[1], double (&)[1]) const {}
+    __device__ __forceinline__ void scrub_carry(double (&)[PPL], double (&)[PPL]) const {}
     __device__ __forceinline__ void on_mask(bool (&on)[NI]) const {
 #pragma unroll
-        for (int c = 0; c < NI; c++) on[c] = true;
+        for (int v = 0; v < NCOL; v++)
+#pragma unroll
+            for (int j = 0; j < PPL; j++) on[v * PPL + j] = real(j);
+    }
+
+    // xl[v] = the left neighbour's last particle of column v (0 at the left wall), xr[v] = the right
+    // neighbour's first particle (0 at the right wall).  In-warp tiles: shuffles.  Wide tiles (L > 32, the
+    // tile is the thread block): shuffles inside each warp, and the two edge lanes of every warp swap their
+    // values through shared memory; the buffer alternates between calls, so one __syncthreads per call.
+    __device__ __forceinline__ void exchange(const double (&Q)[NI], double (&xl)[NCOL], double (&xr)[NCOL]) const {
+        if constexpr (L <= 32) {
+            const bool first = (lt == 0), last = (lt == L - 1);
+#pragma unroll
+            for (int v = 0; v < NCOL; v++) {
+                xl[v] = __shfl_up_sync(0xffffffffu, Q[v * PPL + PPL - 1], 1, L);
+                xr[v] = __shfl_down_sync(0xffffffffu, Q[v * PPL], 1, L);
+                if (first) xl[v] = 0.0;
+                if (last) xr[v] = 0.0;
+            }
+        } else {
+            constexpr int W = L / 32;
+            __shared__ double edge[2][NCOL][2][W];  // [parity][column][first / last particle of the warp][warp]
+            const int wid = lt >> 5, ln = lt & 31;
+#pragma unroll
+            for (int v = 0; v < NCOL; v++) {
+                xl[v] = __shfl_up_sync(0xffffffffu, Q[v * PPL + PPL - 1], 1, 32);
+                xr[v] = __shfl_down_sync(0xffffffffu, Q[v * PPL], 1, 32);
+                if (ln == 0) edge[par][v][0][wid] = Q[v * PPL];
+                if (ln == 31) edge[par][v][1][wid] = Q[v * PPL + PPL - 1];
+            }
+            __syncthreads();
+#pragma unroll
+            for (int v = 0; v < NCOL; v++) {
+                if (ln == 0) xl[v] = (wid > 0) ? edge[par][v][1][wid - 1] : 0.0;
+                if (ln == 31) xr[v] = (wid < W - 1) ? edge[par][v][0][wid + 1] : 0.0;
+            }
+            par ^= 1;
+        }
     }
 
     // Eq.(7) with Eq.(8): p_i' = phi(Dq_{i+1}) - phi(Dq_i), Dq_i = q_i - q_{i-1}; variational:
-    // dp_i' = g(Dq_{i+1}) dDq_{i+1} - g(Dq_i) dDq_i.  Lane i evaluates its LEFT spring; the
-    // right spring's value comes from lane i+1; the last lane also evaluates the wall spring.
+    // dp_i' = g(Dq_{i+1}) dDq_{i+1} - g(Dq_i) dDq_i.  Springs s = 0..PPL of this lane: s = 0 to the left
+    // neighbour (or the left wall), s = PPL to the right neighbour (or the right wall).
     __device__ __forceinline__ void force(const double (&Q)[NI], double (&F)[NI]) const {
-        const bool first = (lt == 0), last = (lt == L - 1);
-        double qL = __shfl_up_sync(0xffffffffu, Q[0], 1, L);
-        if (first) qL = 0.0;
-        const double d = Q[0] - qL;
-        const double phi = fput_phi(prm, d);
-        const double g = fput_g(prm, d);
-        const double dW = -Q[0];  // wall spring of the last particle: q_{N+1} - q_N
-        double phiR = __shfl_down_sync(0xffffffffu, phi, 1, L);
-        double gW = 0.0;
-        if (last) {
-            phiR = fput_phi(prm, dW);
-            gW = fput_g(prm, dW);
+        // all neighbour values first: 2 shuffles per column, none depends on arithmetic
+        double xl[NCOL], xr[NCOL];
+        exchange(Q, xl, xr);
+        double g[PPL + 1], ph[PPL + 1];
+#pragma unroll
+        for (int s = 0; s <= PPL; s++) {
+            const double d = (s == 0) ? Q[0] - xl[0] : (s == PPL) ? xr[0] - Q[PPL - 1] : Q[s] - Q[s - 1];
+            ph[s] = fput_phi(prm, d);
+            g[s] = fput_g(prm, d);
         }
-        F[0] = phiR - phi;
+#pragma unroll
+        for (int j = 0; j < PPL; j++) F[j] = real(j) ? ph[j + 1] - ph[j] : 0.0;
 #pragma unroll
         for (int v = 1; v < NCOL; v++) {
-            double xL = __shfl_up_sync(0xffffffffu, Q[v], 1, L);
-            if (first) xL = 0.0;
-            const double T = g * (Q[v] - xL);
-            double TR = __shfl_down_sync(0xffffffffu, T, 1, L);
-            if (last) TR = gW * (-Q[v]);
-            F[v] = TR - T;
+            const double* X = &Q[v * PPL];
+            double T[PPL + 1];  // T[s] = g_s e_s for the inner springs s = 1..PPL-1
+#pragma unroll
+            for (int s = 1; s < PPL; s++) T[s] = g[s] * (X[s] - X[s - 1]);
+            const double e0 = X[0] - xl[v], eP = xr[v] - X[PPL - 1];
+#pragma unroll
+            for (int j = 0; j < PPL; j++) {
+                double f;
+                if constexpr (PPL == 1) {
+                    f = fma(g[1], eP, -(g[0] * e0));
+                } else {
+                    if (j == 0) f = fma(-g[0], e0, T[1]);
+                    else if (j == PPL - 1) f = fma(g[PPL], eP, -T[PPL - 1]);
+                    else f = T[j + 1] - T[j];
+                }
+                F[v * PPL + j] = real(j) ? f : 0.0;
+            }
         }
     }
 
     __device__ __forceinline__ double dot(int u, int v) const {
-        return tile_sum<L>(fma(q[u], q[v], p[u] * p[v]));
+        double s = 0.0;
+#pragma unroll
+        for (int j = 0; j < PPL; j++) s = fma(q[u * PPL + j], q[v * PPL + j], fma(p[u * PPL + j], p[v * PPL + j], s));
+        return tile_sum<L>(s);
+    }
+    __device__ __forceinline__ void scale(int v, double f) {
+#pragma unroll
+        for (int j = 0; j < PPL; j++) {
+            q[v * PPL + j] *= f;
+            p[v * PPL + j] *= f;
+        }
     }
 
     // w_v <- w_v/|w_v|, lg_v += ln|w_v|
@@ -123,10 +212,8 @@ struct Chain {
 #pragma unroll
         for (int v = 1; v < NCOL; v++) {
             const double s = dot(v, v), ri = fast_rsqrt(s);
-            const double inv = apply ? ri : 1.0;
-            q[v] *= inv;
-            p[v] *= inv;
-            if (want_log && apply) logacc_mul(lg[v], s * ri);
+            scale(v, apply ? ri : 1.0);
+            if (want_log && apply) lg.mul(v, s * ri);
         }
     }
     // modified Gram-Schmidt, right-looking order (see col_kernels.cuh)
@@ -134,16 +221,17 @@ struct Chain {
 #pragma unroll
         for (int v = 1; v < NCOL; v++) {
             const double s = dot(v, v), ri = fast_rsqrt(s);
-            const double inv = apply ? ri : 1.0;
-            q[v] *= inv;
-            p[v] *= inv;
-            if (want_log && apply) logacc_mul(lg[v], s * ri);
+            scale(v, apply ? ri : 1.0);
+            if (want_log && apply) lg.mul(v, s * ri);
 #pragma unroll
             for (int u = v + 1; u < NCOL; u++) {
                 double dt = dot(v, u);
                 if (!apply) dt = 0.0;
-                q[u] = fma(-dt, q[v], q[u]);
-                p[u] = fma(-dt, p[v], p[u]);
+#pragma unroll
+                for (int j = 0; j < PPL; j++) {
+                    q[u * PPL + j] = fma(-dt, q[v * PPL + j], q[u * PPL + j]);
+                    p[u * PPL + j] = fma(-dt, p[v * PPL + j], p[u * PPL + j]);
+                }
             }
         }
     }
@@ -160,18 +248,28 @@ struct Chain {
     template <int IND>
     __device__ __forceinline__ double indicator() const {
         if constexpr (IND == IND_SALI) {
-            const double uq = q[1] + q[K >= 2 ? 2 : 1], up = p[1] + p[K >= 2 ? 2 : 1];
-            const double dq = q[1] - q[K >= 2 ? 2 : 1], dp = p[1] - p[K >= 2 ? 2 : 1];
-            const double sp = sqrt(tile_sum<L>(fma(uq, uq, up * up)));
-            const double sm = sqrt(tile_sum<L>(fma(dq, dq, dp * dp)));
+            constexpr int b = (K >= 2 ? 2 : 1);
+            double sp = 0.0, sm = 0.0;
+#pragma unroll
+            for (int j = 0; j < PPL; j++) {
+                const double uq = q[PPL + j] + q[b * PPL + j], up = p[PPL + j] + p[b * PPL + j];
+                const double dq = q[PPL + j] - q[b * PPL + j], dp = p[PPL + j] - p[b * PPL + j];
+                sp = fma(uq, uq, fma(up, up, sp));
+                sm = fma(dq, dq, fma(dp, dp, sm));
+            }
+            sp = sqrt(tile_sum<L>(sp));
+            sm = sqrt(tile_sum<L>(sm));
             return sp < sm ? sp : sm;
         } else if constexpr (IND == IND_GALI) {
-            double Wq[K], Wp[K];
+            constexpr int M = 2 * PPL;  // this lane's components of a column: (q_j, p_j)
+            double W[K][M];
 #pragma unroll
-            for (int v = 0; v < K; v++) {
-                Wq[v] = q[v + 1];
-                Wp[v] = p[v + 1];
-            }
+            for (int v = 0; v < K; v++)
+#pragma unroll
+                for (int j = 0; j < PPL; j++) {
+                    W[v][2 * j] = q[(v + 1) * PPL + j];
+                    W[v][2 * j + 1] = p[(v + 1) * PPL + j];
+                }
             const double eps = 8.9e-16;
             for (int sweep = 0; sweep < 30; sweep++) {
                 bool rotated = false;
@@ -179,25 +277,36 @@ struct Chain {
                 for (int a = 0; a < K - 1; a++)
 #pragma unroll
                     for (int b = a + 1; b < K; b++) {
-                        const double app = tile_sum<L>(fma(Wq[a], Wq[a], Wp[a] * Wp[a]));
-                        const double aqq = tile_sum<L>(fma(Wq[b], Wq[b], Wp[b] * Wp[b]));
-                        const double apq = tile_sum<L>(fma(Wq[a], Wq[b], Wp[a] * Wp[b]));
+                        double saa = 0.0, sbb = 0.0, sab = 0.0;
+#pragma unroll
+                        for (int c = 0; c < M; c++) {
+                            saa = fma(W[a][c], W[a][c], saa);
+                            sbb = fma(W[b][c], W[b][c], sbb);
+                            sab = fma(W[a][c], W[b][c], sab);
+                        }
+                        const double app = tile_sum<L>(saa), aqq = tile_sum<L>(sbb), apq = tile_sum<L>(sab);
                         const bool rot = fabs(apq) > eps * sqrt(app * aqq);
                         rotated = rotated || rot;
                         const double zeta = (aqq - app) / (2.0 * apq);
                         const double t = copysign(1.0, zeta) / (fabs(zeta) + sqrt(fma(zeta, zeta, 1.0)));
                         const double cs = rot ? rsqrt(fma(t, t, 1.0)) : 1.0, sn = rot ? cs * t : 0.0;
-                        const double xq = Wq[a], yq = Wq[b], xp = Wp[a], yp = Wp[b];
-                        Wq[a] = cs * xq - sn * yq;
-                        Wq[b] = fma(sn, xq, cs * yq);
-                        Wp[a] = cs * xp - sn * yp;
-                        Wp[b] = fma(sn, xp, cs * yp);
+#pragma unroll
+                        for (int c = 0; c < M; c++) {
+                            const double x = W[a][c], y = W[b][c];
+                            W[a][c] = cs * x - sn * y;
+                            W[b][c] = fma(sn, x, cs * y);
+                        }
                     }
-                if (!__any_sync(0xffffffffu, rotated)) break;
+                if (!group_any<L>(rotated)) break;
             }
             double gl = 1.0;
 #pragma unroll
-            for (int v = 0; v < K; v++) gl *= sqrt(tile_sum<L>(fma(Wq[v], Wq[v], Wp[v] * Wp[v])));
+            for (int v = 0; v < K; v++) {
+                double s = 0.0;
+#pragma unroll
+                for (int c = 0; c < M; c++) s = fma(W[v][c], W[v][c], s);
+                gl *= sqrt(tile_sum<L>(s));
+            }
             return gl;
         } else {
             return 0.0;

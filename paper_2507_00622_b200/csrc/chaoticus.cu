@@ -9,6 +9,7 @@
 #include "launch.h"
 
 #include <atomic>
+#include <initializer_list>
 #include <mutex>
 
 namespace {
@@ -20,6 +21,7 @@ thread_local char g_err[512] = "";
 // right after the kernel launch and is handed out again only once that event has completed.  When every
 // slot is busy the call runs without refill (one trajectory per tile: same results, bit for bit).
 std::atomic<int> g_adaptive_refill{1};
+std::atomic<int> g_tune{0};
 constexpr int kQueueSlots = 64, kMaxDevices = 64;
 struct QueuePool {
     unsigned long long* base = nullptr;  // kQueueSlots device counters (cudaMalloc, never freed)
@@ -133,22 +135,50 @@ int dim_of(const chs_problem* pb, int* fput_n) {
     return -1;
 }
 
-int dispatch(const chs::LaunchReq& rq) {
-    int r;
-    if ((r = chs::try_launch_hh(rq)) != -1) return r;
-    if ((r = chs::try_launch_hh_ind(rq)) != -1) return r;
-    if ((r = chs::try_launch_hh_adapt(rq)) != -1) return r;
-    if ((r = chs::try_launch_c3(rq)) != -1) return r;
-    if ((r = chs::try_launch_c3_lyap(rq)) != -1) return r;
-    if ((r = chs::try_launch_fput(rq)) != -1) return r;
-    if ((r = chs::try_launch_fput_adapt(rq)) != -1) return r;
-    if ((r = chs::try_launch_fput_n4(rq)) != -1) return r;
-    if ((r = chs::try_launch_fput_n16(rq)) != -1) return r;
-    if ((r = chs::try_launch_fput_n32(rq)) != -1) return r;
-    if ((r = chs::try_launch_hh_adapt2(rq)) != -1) return r;
-    if ((r = chs::try_launch_c3_more(rq)) != -1) return r;
-    if ((r = chs::try_launch_dp(rq)) != -1) return r;
+// one table per system; FPUT picks the tile class from the chain length (fput_launch.h)
+typedef int (*Launcher)(const chs::LaunchReq&);
+int first_of(const chs::LaunchReq& rq, std::initializer_list<Launcher> ls) {
+    for (Launcher l : ls) {
+        const int r = l(rq);
+        if (r != -1) return r;
+    }
     return -1;
+}
+int dispatch_fput(const chs::LaunchReq& rq) {
+    using namespace chs;
+    const int N = rq.fput_n;
+    int r = -1;
+    switch (N) {  // exact tiles
+        case 4: r = try_launch_fput_n4(rq); break;
+        case 8: r = first_of(rq, {try_launch_fput_n8, try_launch_fput8_more, try_launch_fput8_adapt}); break;
+        case 16: r = try_launch_fput_n16(rq); break;
+        case 32: r = try_launch_fput_n32(rq); break;
+        case 64: r = try_launch_fput_n64(rq); break;
+        default: break;
+    }
+    if (r != -1) return r;
+    if (N < 4) r = try_launch_fput_pad4(rq);
+    else if (N > 4 && N < 8) r = try_launch_fput_pad8(rq);
+    else if (N > 8 && N < 16) r = try_launch_fput_pad16(rq);
+    else if (N > 16 && N < 32) r = try_launch_fput_pad32(rq);
+    else if (N > 32 && N < 64) r = try_launch_fput_pad64(rq);
+    if (r != -1) return r;
+    // wide tiles: longer chains, and what the in-warp classes lack above 32 particles (Lyapunov, adaptive GALI_4)
+    if (N > 32 && N <= 64) return try_launch_fput_wide64(rq);
+    if (N > 64 && N <= 128) return try_launch_fput_wide128(rq);
+    if (N > 128 && N <= 256) return try_launch_fput_wide256(rq);
+    return -1;
+}
+int dispatch(const chs::LaunchReq& rq) {
+    using namespace chs;
+    switch (rq.system) {
+        case CHS_SYS_HENON_HEILES:
+            return first_of(rq, {try_launch_hh, try_launch_hh_ind, try_launch_hh_adapt, try_launch_hh_adapt2});
+        case CHS_SYS_COUPLED3: return first_of(rq, {try_launch_c3, try_launch_c3_lyap, try_launch_c3_more});
+        case CHS_SYS_FPUT: return dispatch_fput(rq);
+        case CHS_SYS_DOUBLE_PENDULUM: return try_launch_dp(rq);
+        default: return -1;
+    }
 }
 
 int finish(int r, const chs::LaunchReq& rq) {
@@ -209,6 +239,7 @@ int run_common(int what, const chs_problem* pb, long long n_ic, double* y, doubl
     rq.tab = make_tab(st->adaptive ? 1.0 : st->h);
     rq.stream = (cudaStream_t)stream;
     rq.info = info;
+    rq.tune = g_tune.load();
     chs::RunArgs& a = rq.args;
     a.n_ic = n_ic;
     a.y = y;
@@ -255,6 +286,10 @@ int chaoticus_version(void) { return CHAOTICUS_VERSION; }
 int chaoticus_set_option(const char* name, int value) {
     if (name && std::strcmp(name, "adaptive_refill") == 0) {
         g_adaptive_refill.store(value != 0 ? 1 : 0);
+        return CHS_OK;
+    }
+    if (name && std::strcmp(name, "tune") == 0) {
+        g_tune.store(value);
         return CHS_OK;
     }
     return fail(CHS_EINVAL, "unknown option '%s'", name ? name : "(null)");

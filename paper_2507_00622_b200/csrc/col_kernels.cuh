@@ -120,8 +120,10 @@ struct Col {
     int lt;          // lane in tile
     double s_lane;   // 1/2 on the orbit lane of a multi-lane tile, else 1
     double q[NI], p[NI];
-    LogAcc lg[CPL];  // deferred-log accumulators of this lane's columns
+    static constexpr bool COLD = false;
+    LogBank<CPL, false> lg;  // deferred-log accumulators of this lane's columns
 
+    __device__ __forceinline__ double dcount() const { return (double)D; }
     __device__ __forceinline__ int col_of(int j) const { return lt * CPL + j; }
     __device__ __forceinline__ bool is_dev(int j) const {
         int c = col_of(j);
@@ -132,14 +134,10 @@ struct Col {
         prm = P;
         lt = (L == 1) ? 0 : (int)(threadIdx.x % L);
         s_lane = (L > 1 && lt == 0) ? 0.5 : 1.0;
-#pragma unroll
-        for (int j = 0; j < CPL; j++) logacc_init(lg[j]);
+        lg.init();
     }
 
-    __device__ __forceinline__ void reset_logs() {
-#pragma unroll
-        for (int j = 0; j < CPL; j++) logacc_init(lg[j]);
-    }
+    __device__ __forceinline__ void reset_logs() { lg.init(); }
 
     __device__ __forceinline__ void load(const double* y, const double* w, long long n_ic, long long ic,
                                          double psign) {
@@ -261,7 +259,7 @@ struct Col {
                 q[j * ND + d] *= inv;
                 p[j * ND + d] *= inv;
             }
-            if (want_log && dev) logacc_mul(lg[j], s * ri);
+            if (want_log && dev) lg.mul(j, s * ri);
         }
     }
 
@@ -297,7 +295,7 @@ struct Col {
                     q[jv * ND + d] = wq[d];
                     p[jv * ND + d] = wp[d];
                 }
-                if (want_log) logacc_mul(lg[jv], r);
+                if (want_log) lg.mul(jv, r);
             }
 #pragma unroll
             for (int j = 0; j < CPL; j++) {
@@ -373,7 +371,7 @@ struct Col {
             for (int j = 0; j < CPL; j++) {
                 if (is_dev(j)) {
                     const long long o = (long long)(col_of(j) - 1) * a.n_ic + ic;
-                    const double lv = logacc_value(lg[j]);
+                    const double lv = lg.value(j);
                     if (a.logacc) a.logacc[o] = bad ? nan("") : a.logacc[o] + lv;
                     if (a.lambda) a.lambda[o] = (bad || elapsed == 0.0) ? nan("") : lv / fabs(elapsed);
                 }
@@ -385,7 +383,8 @@ struct Col {
 // Starting step of the adaptive solver (item 6), any layout S
 template <class S>
 __device__ __forceinline__ double initial_step(const S& s, double interval, double dir, double rtol, double atol) {
-    constexpr int NI = S::NI, L = S::L, D = S::D;
+    constexpr int NI = S::NI, L = S::L;
+    const double D = s.dcount();
     if (interval == 0.0) return 0.0;
     bool on[NI];
     s.on_mask(on);
@@ -480,6 +479,11 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
     double qc[NC], pc[NC], qcn[NC], pcn[NC];  // carried rounding errors of the orbit update
 #pragma unroll
     for (int c = 0; c < NC; c++) qc[c] = pc[c] = 0.0;
+    // "cold" layouts keep the carried words in shared memory between steps ([word][thread]): they are
+    // read and written once per step, and the step itself needs every register
+    constexpr bool COLD = C::COLD && !ADAPT;
+    __shared__ double cold_carry[COLD ? 2 * NC * kMaxTpb : 1];
+    static_assert(!COLD || TPB <= kMaxTpb, "TPB exceeds the cold-state arrays");
 
     if constexpr (!ADAPT) {
         // ---- fixed step: one trajectory per tile, every tile runs the same number of steps -------
@@ -493,10 +497,24 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
         }
         long long slot = 0;
         int cd = a.m, sd = a.sample_every;
+        if constexpr (COLD) {
+#pragma unroll
+            for (int c = 0; c < NC; c++) {
+                cold_carry[c * kMaxTpb + threadIdx.x] = qc[c];
+                cold_carry[(NC + c) * kMaxTpb + threadIdx.x] = pc[c];
+            }
+        }
         for (long long st = 1; st <= a.n_steps; ++st) {
             double F[12][NI];
             dop8_stages<NI, true>(tab, 0.0, 0.0, s.q, s.p, F, force, nohook);
             double qn[NI], pn[NI];
+            if constexpr (COLD) {
+#pragma unroll
+                for (int c = 0; c < NC; c++) {
+                    qc[c] = cold_carry[c * kMaxTpb + threadIdx.x];
+                    pc[c] = cold_carry[(NC + c) * kMaxTpb + threadIdx.x];
+                }
+            }
             dop8_solution<NI, C::NCOMP, true>(tab, 0.0, 0.0, s.q, s.p, F, qn, pn, qc, pc, qcn, pcn);
 #pragma unroll
             for (int c = 0; c < NI; c++) {
@@ -505,14 +523,19 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
             }
 #pragma unroll
             for (int c = 0; c < NC; c++) {
-                qc[c] = qcn[c];
-                pc[c] = pcn[c];
+                if constexpr (COLD) {
+                    cold_carry[c * kMaxTpb + threadIdx.x] = qcn[c];
+                    cold_carry[(NC + c) * kMaxTpb + threadIdx.x] = pcn[c];
+                } else {
+                    qc[c] = qcn[c];
+                    pc[c] = pcn[c];
+                }
             }
             if constexpr (MODE != MODE_NONE) {
                 if (--cd == 0 || st == a.n_steps) {
                     cd = a.m;
                     s.template do_renorm<MODE>(want_log, true);
-                    s.scrub_carry(qc, pc);
+                    if constexpr (!COLD) s.scrub_carry(qc, pc);  // (cold layouts carry orbit words only)
                     if constexpr (IND != IND_NONE) {
                         if (a.sample_every > 0 && --sd == 0) {
                             sd = a.sample_every;
@@ -534,6 +557,13 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
         if constexpr (IND != IND_NONE) ind = s.template indicator<IND>();
         if (!valid) return;
         s.store(a.y, a.w, a.n_ic, ic, bad);
+        if constexpr (COLD) {
+#pragma unroll
+            for (int c = 0; c < NC; c++) {
+                qc[c] = cold_carry[c * kMaxTpb + threadIdx.x];
+                pc[c] = cold_carry[(NC + c) * kMaxTpb + threadIdx.x];
+            }
+        }
         if (a.carry) s.store_carry(a.carry, a.n_ic, ic, qc, pc, bad);
         if constexpr (K > 0) s.store_logs(a, ic, bad, t - a.t0);
         if (s.lt == 0) {
@@ -565,7 +595,7 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
         bool rejected = false, need = true, done = false, first_fetch = true;
         int cd = a.m;
         while (true) {
-            if (__any_sync(0xffffffffu, need)) {
+            if (group_any<L>(need)) {
                 long long nxt = a.n_ic;  // "nothing left"
                 if (a.queue != nullptr) {
                     if (need && s.lt == 0) nxt = (long long)atomicAdd(a.queue, 1ULL);
@@ -593,7 +623,7 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
                 if (got) h_abs = h_init;
                 need = false;
             }
-            if (!__any_sync(0xffffffffu, !done)) break;
+            if (!group_any<L>(!done)) break;
 
             bool active = !done && status == ST_OK && dir * (a.t_end - t) > 0.0;
             if (!rejected) {
@@ -622,7 +652,7 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
             dop8_error_sums<NI>(tab, h, s.q, s.p, qn, pn, F, a.rtol, a.atol, on, S5, S3);
             S5 = tile_sum<L>(S5);
             S3 = tile_sum<L>(S3);
-            const double err = (S5 == 0.0 && S3 == 0.0) ? 0.0 : h_try * S5 * fast_rsqrt((S5 + 0.01 * S3) * (double)C::D);
+            const double err = (S5 == 0.0 && S3 == 0.0) ? 0.0 : h_try * S5 * fast_rsqrt((S5 + 0.01 * S3) * s.dcount());
 
             bool ren = false;
             if (active) {
@@ -658,7 +688,7 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
                 }
             }
             if constexpr (MODE != MODE_NONE) {
-                if (__any_sync(0xffffffffu, ren)) {
+                if (group_any<L>(ren)) {
                     s.template do_renorm<MODE>(want_log, ren);
                     if (ren) s.scrub_carry(qc, pc);
                 }
@@ -666,7 +696,7 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
 
             // trajectories that ended in this iteration: write their results, ask for the next one
             const bool fin = !done && !(status == ST_OK && dir * (a.t_end - t) > 0.0);
-            if (__any_sync(0xffffffffu, fin)) {
+            if (group_any<L>(fin)) {
                 bool bad = !s.finite_all();
                 bad = tile_any<L>(status != ST_OK) || bad;
                 double ind = 0.0;

@@ -42,34 +42,72 @@ struct Tab {
     double h;                 // signed step (fixed) or 1
 };
 
-// ---- tile helpers: a trajectory is owned by L consecutive lanes (L = 1, 2, 4, 8, 16, 32) ----
+// ---- tile helpers: a trajectory is owned by a tile of L consecutive threads -------------------------
+// L = 1, 2, 4, 8, 16, 32: lanes of one warp, shuffles.  L > 32 (wide chains): the tile is the WHOLE thread
+// block (L == blockDim.x, one trajectory per block); the same operations go through shared memory and
+// __syncthreads, and every thread of the block must reach them (run_kernel's control flow is uniform per
+// trajectory, hence per block).  All results are bit-identical on every thread of the tile.
 template <int L>
 __device__ __forceinline__ double tile_bcast(double x, int src_lane_in_tile) {
     if constexpr (L == 1) return x;
-    else return __shfl_sync(0xffffffffu, x, src_lane_in_tile, L);
+    else if constexpr (L <= 32) return __shfl_sync(0xffffffffu, x, src_lane_in_tile, L);
+    else {
+        __shared__ double box;
+        if ((int)threadIdx.x == src_lane_in_tile) box = x;
+        __syncthreads();
+        const double r = box;
+        __syncthreads();
+        return r;
+    }
 }
 template <int L>
 __device__ __forceinline__ long long tile_bcast_ll(long long x, int src_lane_in_tile) {
     if constexpr (L == 1) return x;
-    else return __shfl_sync(0xffffffffu, x, src_lane_in_tile, L);
+    else if constexpr (L <= 32) return __shfl_sync(0xffffffffu, x, src_lane_in_tile, L);
+    else {
+        __shared__ long long box;
+        if ((int)threadIdx.x == src_lane_in_tile) box = x;
+        __syncthreads();
+        const long long r = box;
+        __syncthreads();
+        return r;
+    }
 }
 template <int L>
 __device__ __forceinline__ double tile_sum(double x) {  // butterfly: identical on all lanes
-    if constexpr (L > 1) {
+    if constexpr (L > 1 && L <= 32) {
 #pragma unroll
         for (int d = L / 2; d >= 1; d >>= 1) x += __shfl_xor_sync(0xffffffffu, x, d, L);
+    } else if constexpr (L > 32) {
+        __shared__ double part[L / 32];
+#pragma unroll
+        for (int d = 16; d >= 1; d >>= 1) x += __shfl_xor_sync(0xffffffffu, x, d, 32);
+        if ((threadIdx.x & 31u) == 0u) part[threadIdx.x >> 5] = x;
+        __syncthreads();
+        x = part[0];
+#pragma unroll
+        for (int w = 1; w < L / 32; w++) x += part[w];  // same order on every thread
+        __syncthreads();
     }
     return x;
 }
 template <int L>
 __device__ __forceinline__ bool tile_any(bool b) {
     if constexpr (L == 1) return b;
-    else {
+    else if constexpr (L <= 32) {
         unsigned m = __ballot_sync(0xffffffffu, b);
         unsigned lane = threadIdx.x & 31u;
         unsigned tmask = (L == 32) ? 0xffffffffu : (((1u << L) - 1u) << (lane & ~(unsigned)(L - 1)));
         return (m & tmask) != 0u;
+    } else {
+        return __syncthreads_or(b ? 1 : 0) != 0;
     }
+}
+// "does any thread that shares my control flow want this?": a warp for in-warp tiles, the block for wide ones
+template <int L>
+__device__ __forceinline__ bool group_any(bool b) {
+    if constexpr (L <= 32) return __any_sync(0xffffffffu, b);
+    else return __syncthreads_or(b ? 1 : 0) != 0;
 }
 
 // ---- square roots off the slow path ----------------------------------------------------------
@@ -131,6 +169,53 @@ __device__ __forceinline__ void logacc_mul(LogAcc& a, double r) {  // r > 0, fin
 __device__ __forceinline__ double logacc_value(const LogAcc& a) {
     return fma((double)a.e, 0.693147180559945309417232, log(a.m));
 }
+
+// Threads per block never exceed this (every launcher uses 64 or 128): size of the per-thread
+// "cold state" arrays in shared memory.
+constexpr int kMaxTpb = 128;
+
+// NV deferred-log accumulators per thread.  COLD = false: in registers.  COLD = true: in shared memory
+// ([accumulator][thread]: conflict-free), for kernels whose step needs every register -- the accumulators
+// are touched once per renormalisation, not once per stage.
+template <int NV, bool COLD>
+struct LogBank;
+template <int NV>
+struct LogBank<NV, false> {
+    LogAcc a[NV > 0 ? NV : 1];
+    __device__ __forceinline__ void init() {
+#pragma unroll
+        for (int v = 0; v < NV; v++) logacc_init(a[v]);
+    }
+    __device__ __forceinline__ void mul(int v, double r) { logacc_mul(a[v], r); }
+    __device__ __forceinline__ double value(int v) const { return logacc_value(a[v]); }
+};
+template <int NV>
+struct LogBank<NV, true> {
+    __device__ __forceinline__ static double* m_base() {
+        __shared__ double m[(NV > 0 ? NV : 1) * kMaxTpb];
+        return m;
+    }
+    __device__ __forceinline__ static int* e_base() {
+        __shared__ int e[(NV > 0 ? NV : 1) * kMaxTpb];
+        return e;
+    }
+    __device__ __forceinline__ void init() {
+#pragma unroll
+        for (int v = 0; v < NV; v++) {
+            m_base()[v * kMaxTpb + threadIdx.x] = 1.0;
+            e_base()[v * kMaxTpb + threadIdx.x] = 0;
+        }
+    }
+    __device__ __forceinline__ void mul(int v, double r) {
+        LogAcc t{m_base()[v * kMaxTpb + threadIdx.x], e_base()[v * kMaxTpb + threadIdx.x]};
+        logacc_mul(t, r);
+        m_base()[v * kMaxTpb + threadIdx.x] = t.m;
+        e_base()[v * kMaxTpb + threadIdx.x] = t.e;
+    }
+    __device__ __forceinline__ double value(int v) const {
+        return logacc_value(LogAcc{m_base()[v * kMaxTpb + threadIdx.x], e_base()[v * kMaxTpb + threadIdx.x]});
+    }
+};
 
 // ---- stages -------------------------------------------------------------------------------
 // force(Q, Fout): evaluates the NI force components at the stage coordinates Q.

@@ -1,8 +1,5 @@
-// inst_fput_n32.cu -- FPUT chain, N = 32 (tile of 32 lanes per trajectory): the basic kernel set.
+// inst_fput_n32.cu -- FPUT chain, N = 32 exactly: the basic kernel set (fput_launch.h).
 #include "fput_launch.h"
 namespace chs {
-int try_launch_fput_n32(const LaunchReq& rq) {
-    FPUT_BASIC_SET(32)
-    return -1;
-}
+int try_launch_fput_n32(const LaunchReq& rq) { return fput_basic_set<32, false>(rq); }
 }  // namespace chs

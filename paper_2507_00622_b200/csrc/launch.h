@@ -23,22 +23,34 @@ struct LaunchReq {
     KernelInfo* info;  // non-null: report the launch shape, launch nothing
     // LD: which directions
     int dir_first, n_dirs;
+    int tune;  // development knob (chaoticus_set_option("tune", v)): selects a kernel variant where one exists
 };
 
 // each returns -1 if it has no kernel for the request, else a cudaError_t (0 = success)
 int try_launch_hh(const LaunchReq& rq);
 int try_launch_hh_ind(const LaunchReq& rq);
 int try_launch_hh_adapt(const LaunchReq& rq);
+int try_launch_hh_adapt2(const LaunchReq& rq);
 int try_launch_c3(const LaunchReq& rq);
 int try_launch_c3_lyap(const LaunchReq& rq);
-int try_launch_fput(const LaunchReq& rq);
-int try_launch_fput_adapt(const LaunchReq& rq);
-int try_launch_fput_n4(const LaunchReq& rq);
-int try_launch_fput_n16(const LaunchReq& rq);
-int try_launch_fput_n32(const LaunchReq& rq);
-int try_launch_hh_adapt2(const LaunchReq& rq);
 int try_launch_c3_more(const LaunchReq& rq);
 int try_launch_dp(const LaunchReq& rq);
+// FPUT: by chain length (fput_launch.h "tile classes")
+int try_launch_fput8_more(const LaunchReq& rq);
+int try_launch_fput8_adapt(const LaunchReq& rq);
+int try_launch_fput_n4(const LaunchReq& rq);
+int try_launch_fput_n8(const LaunchReq& rq);
+int try_launch_fput_n16(const LaunchReq& rq);
+int try_launch_fput_n32(const LaunchReq& rq);
+int try_launch_fput_n64(const LaunchReq& rq);
+int try_launch_fput_pad4(const LaunchReq& rq);
+int try_launch_fput_pad8(const LaunchReq& rq);
+int try_launch_fput_pad16(const LaunchReq& rq);
+int try_launch_fput_pad32(const LaunchReq& rq);
+int try_launch_fput_pad64(const LaunchReq& rq);
+int try_launch_fput_wide64(const LaunchReq& rq);
+int try_launch_fput_wide128(const LaunchReq& rq);
+int try_launch_fput_wide256(const LaunchReq& rq);
 
 // Common front part of every launcher: when rq.info is set, report the launch shape of `kern` and
 // return 0 (or a CUDA error); otherwise return -2, meaning "go ahead and launch".

@@ -72,6 +72,7 @@ struct Coupled3 {
 // stiffness g(d) = k + 2 alpha d + 3 beta d^2.  Used by the chain layout (lane = particle).
 struct FputParams {
     double k, al, be, al2, be3;  // al2 = 2 alpha, be3 = 3 beta
+    int np;                      // chain length N (padded tiles: the real length)
 };
 __device__ __forceinline__ double fput_phi(const FputParams& P, double d) {
     return d * fma(d, fma(P.be, d, P.al), P.k);

@@ -32,30 +32,36 @@ def lam_err(lam, ref, T):
     return (np.abs(lam - ref) / np.maximum(np.abs(ref).max(0), 1.0 / T)).max()
 
 
-@pytest.mark.parametrize("N", [4, 16, 32])
+# chain lengths by tile class (fput_launch.h): exact in-warp tiles 4, 16, 32, 64; padded tiles 3, 5, 12, 24,
+# 48 (particles pinned at zero act as the wall); wide tiles (one block per trajectory) 100, 128, 200
+@pytest.mark.parametrize("N", [3, 4, 5, 12, 16, 24, 32, 48, 64, 100, 128, 200])
 def test_fput_other_lengths(chs, orc, N):
-    n_ic = 45          # ragged: 45 tiles of N lanes
+    n_ic = 45 if N <= 32 else (21 if N <= 64 else 7)   # ragged: a few tiles of the last block are padding
+    steps = 1000 if N <= 64 else 400
     prm = W.fput_params(N, 1.0, 0.1, 0.8)
     y0 = W.fput_ics(n_ic, N, seed=3 + N, E=0.1 * N)
     w0 = W.deviation_vectors(n_ic, 4, 2 * N, 50 + N, "orthonormal")
+    info = chs.kernel_info(FPUT, prm, chs.WHAT_GALI, k=4, n_ic=n_ic)
+    assert info["spill_bytes"] == 0
     # plain integration
     yo = y0.copy()
-    orc.integrate_fixed(FPUT, prm, yo, 0.0, 0.05, 1000, precision="f80")
+    orc.integrate_fixed(FPUT, prm, yo, 0.0, 0.05, steps, precision="f80")
     yg = dev(y0)
-    chs.integrate_fixed(FPUT, prm, yg, 0.0, 0.05, 1000)
+    chs.integrate_fixed(FPUT, prm, yg, 0.0, 0.05, steps)
     assert rel_state(yg.cpu().numpy(), yo).max() <= 1e-10
     # GALI_4, fixed step
     yo, wo = y0.copy(), w0.copy()
-    go = orc.gali(FPUT, prm, yo, wo, renorm_every=10, sample_every=10, h=0.05, n_steps=1000, precision="f80")["series"]
+    go = orc.gali(FPUT, prm, yo, wo, renorm_every=10, sample_every=10, h=0.05, n_steps=steps, precision="f80")["series"]
     yg, wg = dev(y0), dev(w0)
-    gg = chs.gali(FPUT, prm, yg, wg, renorm_every=10, sample_every=10, h=0.05, n_steps=1000).cpu().numpy()
+    gg = chs.gali(FPUT, prm, yg, wg, renorm_every=10, sample_every=10, h=0.05, n_steps=steps).cpu().numpy()
     assert go.min() > 1e-9 and np.abs(gg / go - 1).max() <= 1e-8
     assert np.abs(wg.cpu().numpy() - wo).max() <= 1e-9
+    assert rel_state(yg.cpu().numpy(), yo).max() <= 1e-10
     # Lyapunov k = 4 and SALI
     yo, wo = y0.copy(), w0.copy()
-    lo = orc.lyap(FPUT, prm, yo, wo, renorm_every=10, h=0.05, n_steps=1000, precision="f80")["lam"]
-    lg = chs.lyap(FPUT, prm, dev(y0), dev(w0), renorm_every=10, h=0.05, n_steps=1000).cpu().numpy()
-    assert lam_err(lg, lo, 50.0) <= 1e-8
+    lo = orc.lyap(FPUT, prm, yo, wo, renorm_every=10, h=0.05, n_steps=steps, precision="f80")["lam"]
+    lg = chs.lyap(FPUT, prm, dev(y0), dev(w0), renorm_every=10, h=0.05, n_steps=steps).cpu().numpy()
+    assert lam_err(lg, lo, 0.05 * steps) <= 1e-8
     w2 = np.ascontiguousarray(w0[:2])
     so = orc.sali(FPUT, prm, y0.copy(), w2.copy(), renorm_every=5, h=0.05, n_steps=600, precision="f80")["series"]
     sg = chs.sali(FPUT, prm, dev(y0), dev(w2), renorm_every=5, h=0.05, n_steps=600).cpu().numpy()
@@ -64,7 +70,13 @@ def test_fput_other_lengths(chs, orc, N):
     fo, bo = orc.ld(FPUT, prm, y0, 0.0, 0.05, 400, precision="f80")
     f, b = chs.ld(FPUT, prm, dev(y0), 0.0, 0.05, 400)
     assert np.abs(f.cpu().numpy() / fo - 1).max() <= 1e-8 and np.abs(b.cpu().numpy() / bo - 1).max() <= 1e-8
-    # adaptive GALI_4 (the paper's Fig. 3 solver, atol = 1e-8: PAPER.md:129)
+    # adaptive integration and adaptive GALI_4 (the paper's Fig. 3 solver, atol = 1e-8: PAPER.md:129)
+    yo = y0.copy()
+    ro = orc.integrate_adaptive(FPUT, prm, yo, 0.0, 20.0, 1e-10, 1e-10, precision="f80")
+    yg, rep = dev(y0), chs.Report(n_ic, "cuda")
+    chs.integrate_adaptive(FPUT, prm, yg, 0.0, 20.0, 1e-10, 1e-10, report=rep)
+    assert (rep.status.cpu().numpy() == 0).all() and rel_state(yg.cpu().numpy(), yo).max() <= 1e-7
+    assert abs(rep.n_accepted.cpu().numpy().sum() / ro["n_accepted"].sum() - 1) <= 2e-2
     yo, wo = y0.copy(), w0.copy()
     ro = orc.gali(FPUT, prm, yo, wo, renorm_every=1, adaptive=True, t_end=20.0, rtol=1e-8, atol=1e-8, precision="f80")
     rep = chs.Report(n_ic, "cuda")
@@ -73,6 +85,16 @@ def test_fput_other_lengths(chs, orc, N):
     assert (rep.status.cpu().numpy() == 0).all()
     assert np.abs(ga / ro["series"] - 1).max() <= 1e-4
     assert abs(rep.n_accepted.cpu().numpy().sum() / ro["n_accepted"].sum() - 1) <= 2e-2
+
+
+def test_fput_tile_classes_and_limits(chs):
+    """Which tile a chain length runs on (lanes per trajectory), and the longest compiled chain."""
+    lanes = lambda N, what, k, ad=False: chs.kernel_info(FPUT, W.fput_params(N), what, k=k, adaptive=ad, n_ic=10)["lanes"]
+    assert [lanes(N, chs.WHAT_GALI, 4) for N in (3, 4, 5, 8, 9, 16, 33, 64)] == [2, 2, 4, 4, 8, 8, 32, 32]
+    assert [lanes(N, chs.WHAT_GALI, 4, True) for N in (8, 12, 32, 64)] == [8, 16, 32, 64]
+    assert [lanes(N, chs.WHAT_LYAP, 4) for N in (8, 40, 65, 128, 129, 256)] == [8, 64, 128, 128, 256, 256]
+    with pytest.raises(chs.ChaoticusError):
+        lanes(257, chs.WHAT_GALI, 4)
 
 
 def test_fput8_ld_and_adaptive_set(chs, orc):
