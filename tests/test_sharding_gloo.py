@@ -20,10 +20,16 @@ def _worker(rank, world, port, out_dir):
     dist.init_process_group("gloo", rank=rank, world_size=world)
     import bench
     args = types.SimpleNamespace(workload="C2", side=24, n_steps=10)
+    # the rank layout main() takes from the torchrun environment
+    plan = bench.launch_plan(world, os.environ, ["--gpus", str(world)])
+    assert plan == ("run", rank, int(os.environ.get("LOCAL_RANK", "0")), world)
+    assert bench.launch_plan(world + 1, os.environ, [])[0] == "error"    # --gpus contradicts WORLD_SIZE
     wl = bench.workload_inputs(args, rank, world)
-    # the max-over-ranks reduction bench.py applies to its device-timed duration
-    t = torch.tensor([0.5 + rank], dtype=torch.float64)
-    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    # the max-over-ranks reduction bench.py applies to its device-timed duration, and its aggregate
+    tmax = bench.rank_max(0.5 + rank, world)
+    t = torch.tensor([tmax], dtype=torch.float64)
+    agg = bench.aggregate(wl["rk_steps"], world, 3, tmax)
+    assert agg == wl["rk_steps"] * world * 3 / (0.5 + world - 1)
     gathered = [torch.empty_like(torch.from_numpy(wl["y0"])) for _ in range(world)]
     dist.all_gather(gathered, torch.from_numpy(wl["y0"]))
     if rank == 0:
@@ -51,3 +57,33 @@ def test_reference_arm_runs_only_on_rank0(monkeypatch, capsys):
     args = types.SimpleNamespace(side=32, n_steps=5, steps=1, warmup=0, gpus=2)
     assert bench.run_reference(args) is None
     assert capsys.readouterr().out == ""
+
+
+def test_gpus_flag_never_silently_ignored(monkeypatch):
+    """--gpus N outside torchrun re-launches under torch.distributed.run with N ranks; inside torchrun it
+    must equal WORLD_SIZE; bench.py never times one GPU and reports another count."""
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.launch_plan(1, {}, []) == ("run", 0, 0, 1)
+    kind, cmd = bench.launch_plan(8, {}, ["--gpus", "8", "--steps", "2"])
+    assert kind == "spawn" and "--nproc-per-node=8" in cmd and cmd[-4:] == ["--gpus", "8", "--steps", "2"]
+    assert "torch.distributed.run" in cmd and "127.0.0.1" in cmd
+    assert bench.launch_plan(8, {"WORLD_SIZE": "1"}, [])[0] == "error"
+    assert bench.launch_plan(0, {}, [])[0] == "error"
+    assert bench.launch_plan(2, {"WORLD_SIZE": "2", "RANK": "1", "LOCAL_RANK": "1"}, []) == ("run", 1, 1, 2)
+    # no CUDA device here: the spawned ranks must fail loudly, not print a line
+    import subprocess
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "1", "--warmup", "0",
+                        "--configs", ""], capture_output=True, text=True, timeout=600)
+    import torch
+    if not torch.cuda.is_available():
+        assert r.returncode != 0 and '"n_gpus"' not in r.stdout
+
+
+def test_kernel_traffic_comes_from_the_tracked_profile():
+    sys.path.insert(0, ROOT)
+    import bench
+    assert os.path.exists(bench.TRAFFIC_CSV)
+    t = bench.kernel_traffic("C2")
+    assert t is not None and 1e7 < t < 1e8
+    assert bench.kernel_traffic("no-such-workload") is None
