@@ -193,6 +193,12 @@ struct Chain {
         }
     }
 
+    __device__ __forceinline__ void force2(const double (&Qa)[NI], double (&Fa)[NI], const double (&Qb)[NI],
+                                           double (&Fb)[NI]) const {
+        force(Qa, Fa);
+        force(Qb, Fb);
+    }
+
     __device__ __forceinline__ double dot(int u, int v) const {
         double s = 0.0;
 #pragma unroll

@@ -220,41 +220,75 @@ struct LogBank<NV, true> {
 // ---- stages -------------------------------------------------------------------------------
 // force(Q, Fout): evaluates the NI force components at the stage coordinates Q.
 // hook(Int<i>, F): called after stage i's force is available (used by the LD quadrature).
-template <int NI, bool PREMUL, class Force, class Hook>
+//
+// Stage coordinates of stage i (0-based) from the forces of the earlier stages.  A.A has an EMPTY first
+// subdiagonal ((A.A)_{i,i-1} = 0, pinned by tests/test_library_abi.py): Q_i needs F_0 .. F_{i-2} only.
+template <int I, int NI, bool PREMUL>
+__device__ __forceinline__ void dop8_stage_coords(const Tab& tab, double h, double h2, const double (&q)[NI],
+                                                  const double (&p)[NI], const double (&F)[12][NI],
+                                                  double (&Q)[NI]) {
+    static_assert(I >= 1 && I < 12, "stage index");
+#pragma unroll
+    for (int c = 0; c < NI; c++) {
+        if constexpr (PREMUL) {
+            double acc = fma(tab.cs[I], p[c], q[c]);
+            static_for<0, I>([&](auto lc) {
+                constexpr int l = decltype(lc)::value;
+                if constexpr (coef::A2[I][l] != 0.0) acc = fma(tab.a2[I][l], F[l][c], acc);
+            });
+            Q[c] = acc;
+        } else {
+            double base = fma(h * tab.cs[I], p[c], q[c]);
+            if constexpr (I == 1) {
+                Q[c] = base;  // row 2 of A.A is empty
+            } else {
+                double s = tab.a2[I][0] * F[0][c];
+                static_for<1, I>([&](auto lc) {
+                    constexpr int l = decltype(lc)::value;
+                    if constexpr (coef::A2[I][l] != 0.0) s = fma(tab.a2[I][l], F[l][c], s);
+                });
+                Q[c] = fma(h2, s, base);
+            }
+        }
+    }
+}
+
+// The 12 stages.  PAIR = true evaluates them two at a time, (0,1), (2,3), ..., (10,11): stage 2k+1 does
+// not depend on stage 2k (see above), so both stage coordinates are formed first and the two force
+// evaluations -- their neighbour shuffles included -- are independent instruction streams that the
+// scheduler interleaves: twice the instruction-level parallelism exactly where a lane waits on a shuffle
+// and on the short dependent chain of the force.  Same operations in the same order per value: results
+// are bit-identical with PAIR = false.
+template <int NI, bool PREMUL, bool PAIR = true, class Force, class Hook>
 __device__ __forceinline__ void dop8_stages(const Tab& tab, double h, double h2, const double (&q)[NI],
                                             const double (&p)[NI], double (&F)[12][NI], Force&& force,
                                             Hook&& hook) {
-    force(q, F[0]);
-    hook(Int<0>{}, F);
-    static_for<1, 12>([&](auto ic) {
-        constexpr int i = decltype(ic)::value;
-        double Q[NI];
-#pragma unroll
-        for (int c = 0; c < NI; c++) {
-            if constexpr (PREMUL) {
-                double acc = fma(tab.cs[i], p[c], q[c]);
-                static_for<0, i>([&](auto lc) {
-                    constexpr int l = decltype(lc)::value;
-                    if constexpr (coef::A2[i][l] != 0.0) acc = fma(tab.a2[i][l], F[l][c], acc);
-                });
-                Q[c] = acc;
+    if constexpr (PAIR) {
+        static_for<0, 6>([&](auto kc) {
+            constexpr int i0 = 2 * decltype(kc)::value, i1 = i0 + 1;
+            double Qb[NI];
+            dop8_stage_coords<i1, NI, PREMUL>(tab, h, h2, q, p, F, Qb);
+            if constexpr (i0 == 0) {
+                force.pair(q, F[0], Qb, F[i1]);
             } else {
-                double base = fma(h * tab.cs[i], p[c], q[c]);
-                if constexpr (i == 1) {
-                    Q[c] = base;  // row 2 of A.A is empty
-                } else {
-                    double s = tab.a2[i][0] * F[0][c];
-                    static_for<1, i>([&](auto lc) {
-                        constexpr int l = decltype(lc)::value;
-                        if constexpr (coef::A2[i][l] != 0.0) s = fma(tab.a2[i][l], F[l][c], s);
-                    });
-                    Q[c] = fma(h2, s, base);
-                }
+                double Qa[NI];
+                dop8_stage_coords<i0, NI, PREMUL>(tab, h, h2, q, p, F, Qa);
+                force.pair(Qa, F[i0], Qb, F[i1]);
             }
-        }
-        force(Q, F[i]);
-        hook(ic, F);
-    });
+            hook(Int<i0>{}, F);
+            hook(Int<i1>{}, F);
+        });
+    } else {
+        force(q, F[0]);
+        hook(Int<0>{}, F);
+        static_for<1, 12>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            double Q[NI];
+            dop8_stage_coords<i, NI, PREMUL>(tab, h, h2, q, p, F, Q);
+            force(Q, F[i]);
+            hook(ic, F);
+        });
+    }
 }
 
 // 8th-order solution from the stage forces.  The first NCOMP items (the orbit's) are advanced

@@ -88,11 +88,11 @@ inline long long run_grid(const LaunchReq& rq, Kern kern, int tpb, long long n_t
     return blocks;
 }
 
-template <class Sys, int K, int L, int MODE, int IND, bool ADAPT, int TPB, int MINB>
+template <class Sys, int K, int L, int MODE, int IND, bool ADAPT, int TPB, int MINB, bool PAIR = true>
 inline int run_col(const LaunchReq& rq) {
     typename Sys::Params prm;
     if (!Sys::make_params(rq.params, rq.n_params, prm)) return (int)cudaErrorInvalidValue;
-    auto kern = run_kernel<Col<Sys, K, L>, MODE, IND, ADAPT, TPB, MINB>;
+    auto kern = run_kernel<Col<Sys, K, L>, MODE, IND, ADAPT, TPB, MINB, PAIR>;
     const long long n_threads = rq.args.n_ic * L;
     int r = finish_launch(rq, kern, TPB, L, n_threads);
     if (r != -2) return r;

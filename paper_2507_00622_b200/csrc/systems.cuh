@@ -35,6 +35,19 @@ struct HenonHeiles {
         G[0] = -fma(H.xx, x[0], H.xy * x[1]);
         G[1] = -fma(H.xy, x[0], H.yy * x[1]);
     }
+    // G = -(V2'' + s V3''(Q)) x with the products of x formed BEFORE Q is needed: on a multi-lane tile Q
+    // (the orbit's stage coordinates) arrives by shuffle while x is the lane's own column, so only two
+    // dependent FMAs per component follow the shuffle (hess + apply: four levels).
+    //   G0 = -(x0 + Qy (2s x0) + Qx (2s x1)),  G1 = -(x1 + Qx (2s x0) - Qy (2s x1))
+    struct Pre { double u0, u1, x0, x1; };
+    __device__ static __forceinline__ Pre pre(const Params&, const double* x, double s) {
+        const double s2 = 2.0 * s;
+        return Pre{s2 * x[0], s2 * x[1], x[0], x[1]};
+    }
+    __device__ static __forceinline__ void apply_pre(const Params&, const Pre& P, const double* Q, double* G) {
+        G[0] = -fma(Q[1], P.u0, fma(Q[0], P.u1, P.x0));
+        G[1] = -fma(Q[0], P.u0, fma(-Q[1], P.u1, P.x1));
+    }
     __host__ static bool make_params(const double*, int, Params&) { return true; }
 };
 
@@ -59,6 +72,18 @@ struct Coupled3 {
         G[0] = -fma(H.h11, x[0], H.h12 * x[1]);
         G[1] = -fma(H.h12, x[0], fma(H.h22, x[1], H.h23 * x[2]));
         G[2] = -fma(H.h23, x[1], H.h33 * x[2]);
+    }
+    // as HenonHeiles::pre / apply_pre: with t_j = 2 e s x_j and v_j = w_j^2 x_j formed ahead of Q,
+    //   G0 = -(v0 + Q1 t0 + Q0 t1),  G1 = -(v1 + Q0 t0 + Q2 t1 + Q1 t2),  G2 = -(v2 + Q1 t1)
+    struct Pre { double t0, t1, t2, v0, v1, v2; };
+    __device__ static __forceinline__ Pre pre(const Params& P, const double* x, double s) {
+        const double te = 2.0 * P.e * s;
+        return Pre{te * x[0], te * x[1], te * x[2], P.w1s * x[0], P.w2s * x[1], P.w3s * x[2]};
+    }
+    __device__ static __forceinline__ void apply_pre(const Params&, const Pre& R, const double* Q, double* G) {
+        G[0] = -fma(Q[1], R.t0, fma(Q[0], R.t1, R.v0));
+        G[1] = -fma(Q[0], R.t0, fma(Q[2], R.t1, fma(Q[1], R.t2, R.v1)));
+        G[2] = -fma(Q[1], R.t1, R.v2);
     }
     __host__ static bool make_params(const double* p, int n, Params& out) {
         if (n < 4) return false;
