@@ -124,7 +124,20 @@ struct Col {
     LogBank<CPL, false> lg;  // deferred-log accumulators of this lane's columns
 
     __device__ __forceinline__ double dcount() const { return (double)D; }
-    __device__ __forceinline__ int col_of(int j) const { return lt * CPL + j; }
+    // Which column sits in slot j of lane l.  Column 0 (the orbit) is slot 0 of lane 0.  When the other
+    // lanes can hold all K deviation columns (ALONE), lane 0 holds nothing else: its remaining slots are
+    // the tile's idle slots, and every lane needs ONE Hessian per force evaluation (lane 0: V2'' + V3''/2
+    // for the orbit, the others: V2'' + V3'' for both of their columns).  Otherwise columns are dealt in
+    // order, lane 0 mixes the orbit with deviation columns, and two Hessians are formed per lane.
+    static constexpr bool ALONE = (L > 1) && ((L - 1) * CPL >= K);
+    __host__ __device__ static constexpr int col_at(int lane, int j) {
+        if (!ALONE) return lane * CPL + j;
+        if (lane == 0) return j == 0 ? 0 : NCOL;               // NCOL and above: idle slot
+        return 1 + (lane - 1) * CPL + j;
+    }
+    __host__ __device__ static constexpr int owner_of(int c) { return !ALONE ? c / CPL : (c == 0 ? 0 : 1 + (c - 1) / CPL); }
+    __host__ __device__ static constexpr int slot_of(int c) { return !ALONE ? c % CPL : (c == 0 ? 0 : (c - 1) % CPL); }
+    __device__ __forceinline__ int col_of(int j) const { return col_at(lt, j); }
     __device__ __forceinline__ bool is_dev(int j) const {
         int c = col_of(j);
         return c >= 1 && c < NCOL;
@@ -232,15 +245,20 @@ struct Col {
 #pragma unroll
             for (int d = 0; d < ND; d++) Qo[d] = tile_bcast<L>(Q[d], 0);
             Sys::apply_pre(prm, P, Qo, &F[0]);
-        } else {  // several columns per lane: one Hessian serves them (fewer instructions; measured faster)
+        } else {  // several columns per lane: a Hessian serves them (fewer instructions; measured faster)
             double Qo[ND];
 #pragma unroll
             for (int d = 0; d < ND; d++) Qo[d] = tile_bcast<L>(Q[d], 0);
             const typename Sys::Hess H0 = Sys::hess(prm, Qo, s_lane);
             Sys::apply(H0, &Q[0], &F[0]);
-            const typename Sys::Hess H1 = Sys::hess(prm, Qo, 1.0);
+            if constexpr (ALONE) {  // lane 0's other slots are idle: the same Hessian for every slot of a lane
 #pragma unroll
-            for (int j = 1; j < CPL; j++) Sys::apply(H1, &Q[j * ND], &F[j * ND]);
+                for (int j = 1; j < CPL; j++) Sys::apply(H0, &Q[j * ND], &F[j * ND]);
+            } else {
+                const typename Sys::Hess H1 = Sys::hess(prm, Qo, 1.0);
+#pragma unroll
+                for (int j = 1; j < CPL; j++) Sys::apply(H1, &Q[j * ND], &F[j * ND]);
+            }
         }
     }
     // two independent force evaluations (dop8_stages PAIR)
@@ -253,7 +271,7 @@ struct Col {
     // value of component cc (0..N-1) of column `col` (compile-time), on every lane of the tile
     template <int COL>
     __device__ __forceinline__ double gather(int cc) const {
-        constexpr int owner = COL / CPL, j = COL % CPL;
+        constexpr int owner = owner_of(COL), j = slot_of(COL);
         const double v = (cc < ND) ? q[j * ND + cc] : p[j * ND + (cc - ND)];
         return tile_bcast<L>(v, owner);
     }
@@ -285,7 +303,7 @@ struct Col {
     __device__ __forceinline__ void mgs(bool want_log, bool apply) {
         static_for<1, NCOL>([&](auto vc) {
             constexpr int v = decltype(vc)::value;
-            constexpr int owner = v / CPL, jv = v % CPL;
+            constexpr int owner = owner_of(v), jv = slot_of(v);
             double wq[ND], wp[ND];
             double s = 0.0;
 #pragma unroll
