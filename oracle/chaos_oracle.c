@@ -771,6 +771,49 @@ int orc_ld(int sys, const double *params, long long n_ic, const double *y0, doub
     return ORC_OK;
 }
 
+/* Lagrangian descriptors of an initial condition AND of its 2n axis neighbours (PAPER.md:57-58:
+ * "Generation of neighbouring trajectories for the calculation of the chaos indicators based on
+ * Lagrangian Descriptors").  For every IC x0 the members are
+ *   m = 0: x0;   m = 1 + 2i: x0 + sigma e_i;   m = 2 + 2i: x0 - sigma e_i,   i = 0..n-1,
+ * e_i the unit vector of phase-space component i in the library's ordering (q_1..q_N, p_1..p_N).
+ * Each member's forward / backward LD is orc_ld of the displaced initial condition -- a plain loop.
+ * ld_fwd, ld_bwd: [1+2n][n_ic] (row = member), either may be NULL.
+ * diff_fwd, diff_bwd: [2n][n_ic] or NULL, the raw differences |M(x0 +- sigma e_i) - M(x0)|
+ * (row 2i: +, row 2i+1: -).  The LD-based chaos indicators of refs [11,26,68,10,31] are built from
+ * these differences; their final scalar formulas are only CITED by the paper, not printed,
+ * and are therefore not restated here (R19): this function stops at what the paper defines. */
+int orc_ld_neighbours(int sys, const double *params, long long n_ic, const double *y0, double sigma,
+                      double t0, double h, long long n_steps, double *ld_fwd, double *ld_bwd,
+                      double *diff_fwd, double *diff_bwd, int n_threads)
+{
+    int n = orc_dim(sys, params);
+    if (n < 0 || n_ic < 0 || !y0 || !(h > 0) || n_steps < 0 || !(sigma >= 0)) return ORC_EINVAL;
+    if ((diff_fwd && !ld_fwd) || (diff_bwd && !ld_bwd)) return ORC_EINVAL;
+    double *yd = malloc(sizeof(double) * (size_t)n * (size_t)(n_ic > 0 ? n_ic : 1));
+    if (!yd) return ORC_EINVAL;
+    int rc = ORC_OK;
+    for (int m = 0; m < 1 + 2 * n && rc == ORC_OK; m++) {
+        memcpy(yd, y0, sizeof(double) * (size_t)n * (size_t)n_ic);
+        if (m > 0) {
+            int i = (m - 1) / 2;
+            double delta = ((m - 1) % 2 == 0) ? sigma : -sigma;
+            for (long long ic = 0; ic < n_ic; ic++) yd[(long long)i * n_ic + ic] = y0[(long long)i * n_ic + ic] + delta;
+        }
+        rc = orc_ld(sys, params, n_ic, yd, t0, h, n_steps, ld_fwd ? ld_fwd + (long long)m * n_ic : NULL,
+                    ld_bwd ? ld_bwd + (long long)m * n_ic : NULL, n_threads);
+    }
+    free(yd);
+    if (rc != ORC_OK) return rc;
+    for (int pass = 0; pass < 2; pass++) {
+        const double *M = pass == 0 ? ld_fwd : ld_bwd;
+        double *D = pass == 0 ? diff_fwd : diff_bwd;
+        if (!D) continue;
+        for (int r = 0; r < 2 * n; r++)
+            for (long long ic = 0; ic < n_ic; ic++) D[(long long)r * n_ic + ic] = fabs(M[(long long)(r + 1) * n_ic + ic] - M[ic]);
+    }
+    return ORC_OK;
+}
+
 /* ------------------------------------------------------------------------------------
  * Small single-trajectory entry points used only by the pins.
  * ---------------------------------------------------------------------------------- */

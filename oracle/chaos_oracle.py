@@ -52,6 +52,9 @@ def _lib(precision):
         lib.orc_ld.restype = C.c_int
         lib.orc_ld.argtypes = [C.c_int, _dp, C.c_longlong, _dp, C.c_double, C.c_double, C.c_longlong, _dp, _dp,
                                C.c_int]
+        lib.orc_ld_neighbours.restype = C.c_int
+        lib.orc_ld_neighbours.argtypes = [C.c_int, _dp, C.c_longlong, _dp, C.c_double, C.c_double, C.c_double,
+                                          C.c_longlong, _dp, _dp, _dp, _dp, C.c_int]
         lib.orc_rhs.argtypes = [C.c_int, _dp, C.c_int, _dp, _dp]
         lib.orc_energy.argtypes = [C.c_int, _dp, C.c_longlong, _dp, _dp]
         lib.orc_step.argtypes = [C.c_int, _dp, C.c_int, _dp, C.c_double, _dp, C.c_double, C.c_double, _dp]
@@ -161,6 +164,26 @@ def ld(system, params, y0, t0, h, n_steps, *, forward=True, backward=True, preci
     if rc != 0:
         raise ValueError("orc_ld: invalid arguments")
     return f, b
+
+
+def ld_neighbours(system, params, y0, sigma, t0, h, n_steps, *, forward=True, backward=True, diffs=True,
+                  precision="f64", threads=None):
+    """LD of every IC and of its 2n axis neighbours x0 +- sigma e_i (rows: centre, +e_0, -e_0, +e_1, ...).
+    Returns dict(fwd [1+2n, n_ic], bwd, diff_fwd [2n, n_ic], diff_bwd); absent ones are None."""
+    lib = _lib(precision)
+    pr = _params(params)
+    n = dim(system, pr)
+    n_ic = y0.shape[1]
+    _chk(y0, (n, n_ic), "y0")
+    f = np.empty((1 + 2 * n, n_ic)) if forward else None
+    b = np.empty((1 + 2 * n, n_ic)) if backward else None
+    df = np.empty((2 * n, n_ic)) if (forward and diffs) else None
+    db = np.empty((2 * n, n_ic)) if (backward and diffs) else None
+    rc = lib.orc_ld_neighbours(system, _p(pr), n_ic, _p(y0), sigma, t0, h, n_steps, _p(f), _p(b), _p(df), _p(db),
+                               threads or default_threads())
+    if rc != 0:
+        raise ValueError("orc_ld_neighbours: invalid arguments")
+    return dict(fwd=f, bwd=b, diff_fwd=df, diff_bwd=db)
 
 
 # ---- single-trajectory helpers used by the pins --------------------------------------------

@@ -307,3 +307,59 @@ def test_invalid_arguments(orc):
         orc.integrate_adaptive(HH, None, y, 0.0, 1.0, 0.0, 1e-9)         # rtol = 0
     out = orc.integrate_fixed(HH, None, np.zeros((4, 0)), 0.0, 0.01, 10)  # empty ensemble: no-op
     assert out["status"].size == 0
+
+
+# ----------------------------------------------------------------------------- LD neighbours
+def test_ld_neighbours_closed_form_and_ordering(orc):
+    """Equal frequencies, no coupling: |f| = |y| is constant along an orbit, so M(x) = tau |x| for EVERY
+    initial condition, on or off the energy surface.  The members' LDs and the raw differences are then
+    analytic: M(x0 +- sigma e_i) = tau |x0 +- sigma e_i|.  The components of x0 are all distinct, so a
+    wrong component, a wrong sign or a wrong row order changes the expected value."""
+    prm = np.array([1.0, 1.0, 1.0, 0.0])
+    rng = np.random.default_rng(11)
+    y0 = np.ascontiguousarray(rng.uniform(0.2, 1.0, size=(6, 9)) * rng.choice([-1.0, 1.0], size=(6, 9)))
+    sigma, h, ns = 0.05, 0.01, 800
+    tau = h * ns
+    r = orc.ld_neighbours(C3, prm, y0, sigma, 0.0, h, ns, precision="f64")
+    assert r["fwd"].shape == (13, 9) and r["diff_fwd"].shape == (12, 9)
+    M0 = tau * np.linalg.norm(y0, axis=0)
+    assert np.abs(r["fwd"][0] / M0 - 1).max() <= 1e-12 and np.abs(r["bwd"][0] / M0 - 1).max() <= 1e-12
+    for i in range(6):
+        for s, row in ((+1.0, 1 + 2 * i), (-1.0, 2 + 2 * i)):
+            yd = y0.copy()
+            yd[i] += s * sigma
+            Md = tau * np.linalg.norm(yd, axis=0)
+            assert np.abs(r["fwd"][row] / Md - 1).max() <= 1e-12, (i, s)
+            assert np.abs(r["bwd"][row] / Md - 1).max() <= 1e-12, (i, s)
+            assert np.abs(r["diff_fwd"][row - 1] - np.abs(Md - M0)).max() <= 1e-11, (i, s)
+            assert np.abs(r["diff_bwd"][row - 1] - np.abs(Md - M0)).max() <= 1e-11, (i, s)
+    # central difference of the members -> the analytic gradient tau x_i / |x|, error O(sigma^2)
+    grad = (r["fwd"][1::2] - r["fwd"][2::2]) / (2 * sigma)
+    exact = tau * y0 / np.linalg.norm(y0, axis=0)
+    assert np.abs(grad - exact).max() <= 2.0 * tau * sigma ** 2
+
+
+def test_ld_neighbours_sigma_zero_and_generator(orc):
+    """sigma = 0: every member is the centre, all differences vanish exactly.  sigma > 0 on a system whose
+    components are not interchangeable (Henon-Heiles): every member equals the LD of the displaced IC built
+    here with numpy."""
+    y0 = wl.hh_grid(0.125, 5, 4)
+    r0 = orc.ld_neighbours(HH, None, y0, 0.0, 0.0, 0.01, 300, precision="f64")
+    assert (r0["fwd"] == r0["fwd"][0]).all() and (r0["bwd"] == r0["bwd"][0]).all()
+    assert (r0["diff_fwd"] == 0).all() and (r0["diff_bwd"] == 0).all()
+    f0, b0 = orc.ld(HH, None, y0, 0.0, 0.01, 300, precision="f64")
+    assert (r0["fwd"][0] == f0).all() and (r0["bwd"][0] == b0).all()
+    sigma = 1e-3
+    r = orc.ld_neighbours(HH, None, y0, sigma, 0.0, 0.01, 300, precision="f64")
+    for m in range(1, 9):
+        yd = y0.copy()
+        yd[(m - 1) // 2] += sigma if (m - 1) % 2 == 0 else -sigma
+        fd, bd = orc.ld(HH, None, yd, 0.0, 0.01, 300, precision="f64")
+        assert (r["fwd"][m] == fd).all() and (r["bwd"][m] == bd).all(), m
+        assert (r["diff_fwd"][m - 1] == np.abs(fd - f0)).all()
+    # the differences shrink linearly with sigma (M is smooth over t = 3)
+    r2 = orc.ld_neighbours(HH, None, y0, sigma / 2, 0.0, 0.01, 300, precision="f64")
+    ratio = r["diff_fwd"] / r2["diff_fwd"]
+    assert np.median(np.abs(ratio - 2.0)) <= 0.01 and np.abs(ratio - 2.0).max() <= 0.25   # (small gradients: O(sigma^2) shows)
+    with pytest.raises(ValueError):
+        orc.ld_neighbours(HH, None, y0, -1.0, 0.0, 0.01, 10)
