@@ -141,6 +141,21 @@ int chaoticus_gali(const chs_problem* pb, long long n_ic, double* y, double* w, 
 int chaoticus_ld(const chs_problem* pb, long long n_ic, const double* y0, double t0, double h,
                  long long n_steps, double* ld_fwd, double* ld_bwd, void* stream);
 
+/* Neighbouring trajectories for the LD-based chaos indicators: for every
+ * IC x0 the 1 + 2n members  m = 0: x0;  m = 1 + 2i: x0 + sigma e_i;  m = 2 + 2i: x0 - sigma e_i
+ * (e_i: unit vector of phase-space component i in the ordering of y) are generated ON THE DEVICE and
+ * integrated in ONE launch together with the centres, forward and backward, as chaoticus_ld does.
+ *  y0                DEVICE [n][n_ic], not modified;  sigma >= 0
+ *  ld_fwd, ld_bwd    DEVICE [1+2n][n_ic] (row = member), either may be NULL
+ *  diff_fwd/_bwd     DEVICE [2n][n_ic] or NULL: the raw differences |M(x0 +- sigma e_i) - M(x0)|
+ *                    (row 2i: +, row 2i+1: -), formed on the same stream right after the LD launch;
+ *                    a difference array needs the LD array of its direction.
+ * The final scalar indicators of refs [11,26,68,10,31] are only cited by the paper, not printed; this call
+ * returns what the paper defines -- the members' LDs and their differences (R19). */
+int chaoticus_ld_neighbours(const chs_problem* pb, long long n_ic, const double* y0, double sigma, double t0,
+                            double h, long long n_steps, double* ld_fwd, double* ld_bwd, double* diff_fwd,
+                            double* diff_bwd, void* stream);
+
 /* PAPER.md:51-52 (solvers 5, 6): 1 <= k <= n vectors, modified Gram-Schmidt every
  * renorm_every accepted steps and at the end (orthonormalised once on entry),
  * S_v += ln r_vv.  lambda DEVICE [k][n_ic] = this run's sums / |elapsed time| (growth rates per
@@ -153,6 +168,9 @@ int chaoticus_lyap(const chs_problem* pb, long long n_ic, double* y, double* w, 
  * They allocate device scratch, copy in, run on an internal stream, copy out and synchronise. */
 int chaoticus_ld_host(const chs_problem* pb, long long n_ic, const double* y0, double t0, double h,
                       long long n_steps, double* ld_fwd, double* ld_bwd);
+int chaoticus_ld_neighbours_host(const chs_problem* pb, long long n_ic, const double* y0, double sigma, double t0,
+                                 double h, long long n_steps, double* ld_fwd, double* ld_bwd, double* diff_fwd,
+                                 double* diff_bwd);
 int chaoticus_sali_host(const chs_problem* pb, long long n_ic, double* y, double* w, const chs_stepper* st,
                         int renorm_every, int sample_every, double* sali, double* lognorm,
                         const chs_report* rep);

@@ -23,7 +23,7 @@ ST_OK, ST_NONFINITE, ST_UNDERFLOW, ST_MAXSTEPS = 0, 1, 2, 3
 EXPORTS = [
     "chaoticus_version", "chaoticus_last_error", "chaoticus_dim", "chaoticus_n_samples",
     "chaoticus_integrate_fixed", "chaoticus_integrate_adaptive", "chaoticus_sali", "chaoticus_gali",
-    "chaoticus_ld", "chaoticus_lyap", "chaoticus_ld_host", "chaoticus_sali_host", "chaoticus_gali_host",
+    "chaoticus_ld", "chaoticus_ld_neighbours", "chaoticus_ld_neighbours_host", "chaoticus_lyap", "chaoticus_ld_host", "chaoticus_sali_host", "chaoticus_gali_host",
     "chaoticus_lyap_host", "chaoticus_integrate_host", "chaoticus_kernel_info", "chaoticus_set_option",
 ]
 
@@ -63,6 +63,8 @@ def _load():
     lib.chaoticus_sali.argtypes = [PP, ll, vp, vp, SP, i, i, vp, vp, RP, vp]
     lib.chaoticus_gali.argtypes = [PP, ll, vp, vp, i, SP, i, i, vp, vp, RP, vp]
     lib.chaoticus_ld.argtypes = [PP, ll, vp, dbl, dbl, ll, vp, vp, vp]
+    lib.chaoticus_ld_neighbours.argtypes = [PP, ll, vp, dbl, dbl, dbl, ll, vp, vp, vp, vp, vp]
+    lib.chaoticus_ld_neighbours_host.argtypes = [PP, ll, vp, dbl, dbl, dbl, ll, vp, vp, vp, vp]
     lib.chaoticus_lyap.argtypes = [PP, ll, vp, vp, i, SP, i, vp, vp, RP, vp]
     lib.chaoticus_ld_host.argtypes = [PP, ll, vp, dbl, dbl, ll, vp, vp]
     lib.chaoticus_sali_host.argtypes = [PP, ll, vp, vp, SP, i, i, vp, vp, RP]
@@ -238,6 +240,25 @@ def ld(system, params, y0, t0, h, n_steps, *, forward=True, backward=True, out_f
     return f, b
 
 
+def ld_neighbours(system, params, y0, sigma, t0, h, n_steps, *, forward=True, backward=True, diffs=True,
+                  out_fwd=None, out_bwd=None):
+    """LD of every IC and of its 2n axis neighbours x0 +- sigma e_i, generated on the device.
+    Returns dict(fwd [1+2n, n_ic], bwd, diff_fwd [2n, n_ic], diff_bwd); absent ones are None."""
+    pb = _problem(system, params)
+    n = _dim(pb)
+    n_ic = y0.shape[1]
+    new = lambda rows: torch.empty((rows, n_ic), dtype=torch.float64, device=y0.device)
+    f = (out_fwd if out_fwd is not None else new(1 + 2 * n)) if forward else None
+    b = (out_bwd if out_bwd is not None else new(1 + 2 * n)) if backward else None
+    df = new(2 * n) if (forward and diffs) else None
+    db = new(2 * n) if (backward and diffs) else None
+    _check(_lib.chaoticus_ld_neighbours(C.byref(pb), n_ic, _dev(y0, (n, n_ic), "y0"), sigma, t0, h, int(n_steps),
+                                        _dev(f, (1 + 2 * n, n_ic), "ld_fwd"), _dev(b, (1 + 2 * n, n_ic), "ld_bwd"),
+                                        _dev(df, (2 * n, n_ic), "diff_fwd"), _dev(db, (2 * n, n_ic), "diff_bwd"),
+                                        _stream()))
+    return dict(fwd=f, bwd=b, diff_fwd=df, diff_bwd=db)
+
+
 # ---- host-buffer forms ------------------------------------------------------------------------
 def _host(a, shape, name, dtype=np.float64):
     if a is None:
@@ -258,6 +279,17 @@ def ld_host(system, params, y0, t0, h, n_steps, ld_fwd=None, ld_bwd=None):
     n_ic = y0.shape[1]
     _check(_lib.chaoticus_ld_host(C.byref(pb), n_ic, _host(y0, (n, n_ic), "y0"), t0, h, int(n_steps),
                                   _host(ld_fwd, (n_ic,), "ld_fwd"), _host(ld_bwd, (n_ic,), "ld_bwd")))
+
+
+def ld_neighbours_host(system, params, y0, sigma, t0, h, n_steps, ld_fwd=None, ld_bwd=None, diff_fwd=None,
+                       diff_bwd=None):
+    pb = _problem(system, params)
+    n = _dim(pb)
+    n_ic = y0.shape[1]
+    _check(_lib.chaoticus_ld_neighbours_host(
+        C.byref(pb), n_ic, _host(y0, (n, n_ic), "y0"), sigma, t0, h, int(n_steps),
+        _host(ld_fwd, (1 + 2 * n, n_ic), "ld_fwd"), _host(ld_bwd, (1 + 2 * n, n_ic), "ld_bwd"),
+        _host(diff_fwd, (2 * n, n_ic), "diff_fwd"), _host(diff_bwd, (2 * n, n_ic), "diff_bwd")))
 
 
 def sali_host(system, params, y, w, sali_out, *, renorm_every=1, sample_every=0, lognorm=None, report=None,

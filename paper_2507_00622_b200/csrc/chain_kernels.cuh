@@ -67,6 +67,15 @@ struct Chain {
             }
         }
     }
+    __device__ __forceinline__ void displace(int comp, double delta, double psign) {
+#pragma unroll
+        for (int j = 0; j < PPL; j++) {
+            const int pi = lt * PPL + j;
+            if (!real(j)) continue;  // (a padded slot's index collides with a momentum component)
+            if (comp == pi) q[j] += delta;
+            if (comp == np + pi) p[j] += psign * delta;
+        }
+    }
     __device__ __forceinline__ void store(double* y, double* w, long long n_ic, long long ic, bool bad) const {
         const int n = 2 * np;
 #pragma unroll

@@ -84,6 +84,14 @@ void release_after_launch(const QueueLease& l, cudaStream_t stream) {
     P.pending[l.slot] = false;
 }
 
+// raw differences |M(x0 +- sigma e_i) - M(x0)| of the members' LDs: ld [1+2n][n_ic] ->
+// diff [2n][n_ic].  A stencil over values the LD launch has just written (same stream).
+__global__ void ld_diff_kernel(const double* __restrict__ ld, double* __restrict__ diff, long long n_ic, int n_rows) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_ic * n_rows) return;
+    diff[i] = fabs(ld[i + n_ic] - ld[i % n_ic]);
+}
+
 int fail(int rc, const char* fmt, ...) {
     va_list ap;
     va_start(ap, fmt);
@@ -346,7 +354,8 @@ int chaoticus_lyap(const chs_problem* pb, long long n_ic, double* y, double* w, 
 }
 
 static int ld_common(const chs_problem* pb, long long n_ic, const double* y0, double t0, double h,
-                     long long n_steps, double* ld_fwd, double* ld_bwd, void* stream, chs::KernelInfo* info) {
+                     long long n_steps, double* ld_fwd, double* ld_bwd, void* stream, chs::KernelInfo* info,
+                     int n_members = 1, double sigma = 0.0) {
     (void)t0;  // autonomous systems: time is bookkeeping only
     int fput_n = 0;
     const int n = dim_of(pb, &fput_n);
@@ -374,6 +383,8 @@ static int ld_common(const chs_problem* pb, long long n_ic, const double* y0, do
     rq.args.n_steps = n_steps;
     rq.args.ld_fwd = ld_fwd;
     rq.args.ld_bwd = ld_bwd;
+    rq.args.n_members = n_members;
+    rq.args.sigma = sigma;
     rq.dir_first = ld_fwd ? 0 : 1;
     rq.n_dirs = (info || (ld_fwd && ld_bwd)) ? 2 : 1;
     if (info) rq.dir_first = 0;
@@ -384,6 +395,25 @@ static int ld_common(const chs_problem* pb, long long n_ic, const double* y0, do
 int chaoticus_ld(const chs_problem* pb, long long n_ic, const double* y0, double t0, double h, long long n_steps,
                  double* ld_fwd, double* ld_bwd, void* stream) {
     return ld_common(pb, n_ic, y0, t0, h, n_steps, ld_fwd, ld_bwd, stream, nullptr);
+}
+
+int chaoticus_ld_neighbours(const chs_problem* pb, long long n_ic, const double* y0, double sigma, double t0,
+                            double h, long long n_steps, double* ld_fwd, double* ld_bwd, double* diff_fwd,
+                            double* diff_bwd, void* stream) {
+    const int n = dim_of(pb, nullptr);
+    if (n < 0) return fail(CHS_EINVAL, "unknown system or bad params");
+    if (!(sigma >= 0.0) || !std::isfinite(sigma)) return fail(CHS_EINVAL, "ld_neighbours: sigma must be finite and >= 0");
+    if ((diff_fwd && !ld_fwd) || (diff_bwd && !ld_bwd))
+        return fail(CHS_EINVAL, "ld_neighbours: differences need the LD array of the same direction");
+    const int rc = ld_common(pb, n_ic, y0, t0, h, n_steps, ld_fwd, ld_bwd, stream, nullptr, 1 + 2 * n, sigma);
+    if (rc != CHS_OK || n_ic == 0) return rc;
+    const long long total = n_ic * 2LL * n;
+    const unsigned blocks = (unsigned)((total + 255) / 256);
+    if (diff_fwd) ld_diff_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(ld_fwd, diff_fwd, n_ic, 2 * n);
+    if (diff_bwd) ld_diff_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(ld_bwd, diff_bwd, n_ic, 2 * n);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(CHS_ECUDA, "CUDA error %d: %s", (int)e, cudaGetErrorString(e));
+    return CHS_OK;
 }
 
 int chaoticus_kernel_info(const chs_problem* pb, int what, int k, int adaptive, long long n_ic, int* info5) {
@@ -545,6 +575,41 @@ int chaoticus_ld_host(const chs_problem* pb, long long n_ic, const double* y0, d
     }
     if (ld_fwd) CK(cudaMemcpyAsync(ld_fwd, df.p, bo, cudaMemcpyDeviceToHost, stream));
     if (ld_bwd) CK(cudaMemcpyAsync(ld_bwd, db.p, bo, cudaMemcpyDeviceToHost, stream));
+    CK(cudaStreamSynchronize(stream));
+    return CHS_OK;
+}
+
+int chaoticus_ld_neighbours_host(const chs_problem* pb, long long n_ic, const double* y0, double sigma, double t0,
+                                 double h, long long n_steps, double* ld_fwd, double* ld_bwd, double* diff_fwd,
+                                 double* diff_bwd) {
+    cudaStream_t stream = nullptr;
+    const int n = dim_of(pb, nullptr);
+    if (n < 0) return fail(CHS_EINVAL, "unknown system or bad params");
+    if (n_ic < 0) return fail(CHS_EINVAL, "n_ic < 0");
+    if ((diff_fwd && !ld_fwd) || (diff_bwd && !ld_bwd))
+        return fail(CHS_EINVAL, "ld_neighbours: differences need the LD array of the same direction");
+    if (n_ic == 0 || (!ld_fwd && !ld_bwd)) return CHS_OK;
+    if (!y0) return fail(CHS_EINVAL, "y0 is NULL");
+    DevBuf dy, df, db, ddf, ddb;
+    const size_t by = sizeof(double) * (size_t)n * n_ic, bo = sizeof(double) * (size_t)(1 + 2 * n) * n_ic,
+                 bd = sizeof(double) * (size_t)(2 * n) * n_ic;
+    CK(host_stream(&stream));
+    CK(dy.alloc(by, stream));
+    if (ld_fwd) CK(df.alloc(bo, stream));
+    if (ld_bwd) CK(db.alloc(bo, stream));
+    if (diff_fwd) CK(ddf.alloc(bd, stream));
+    if (diff_bwd) CK(ddb.alloc(bd, stream));
+    CK(cudaMemcpyAsync(dy.p, y0, by, cudaMemcpyHostToDevice, stream));
+    int rc = chaoticus_ld_neighbours(pb, n_ic, (const double*)dy.p, sigma, t0, h, n_steps, (double*)df.p, (double*)db.p,
+                                     (double*)ddf.p, (double*)ddb.p, stream);
+    if (rc) {
+        cudaStreamSynchronize(stream);
+        return rc;
+    }
+    if (ld_fwd) CK(cudaMemcpyAsync(ld_fwd, df.p, bo, cudaMemcpyDeviceToHost, stream));
+    if (ld_bwd) CK(cudaMemcpyAsync(ld_bwd, db.p, bo, cudaMemcpyDeviceToHost, stream));
+    if (diff_fwd) CK(cudaMemcpyAsync(diff_fwd, ddf.p, bd, cudaMemcpyDeviceToHost, stream));
+    if (diff_bwd) CK(cudaMemcpyAsync(diff_bwd, ddb.p, bd, cudaMemcpyDeviceToHost, stream));
     CK(cudaStreamSynchronize(stream));
     return CHS_OK;
 }

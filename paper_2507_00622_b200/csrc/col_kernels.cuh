@@ -55,6 +55,10 @@ struct RunArgs {
     const double* y0;
     double* ld_fwd;
     double* ld_bwd;
+    // LD of neighbouring initial conditions: members per IC (1 = the IC itself only;
+    // 1 + 2n = centre and x0 +- sigma e_i), outputs are [member][ic]
+    int n_members;
+    double sigma;
     // adaptive runs: work queue for lane refill (device counter, zeroed before the launch), or null
     unsigned long long* queue;
 };
@@ -170,6 +174,16 @@ struct Col {
                 q[j * ND + d] = qq;
                 p[j * ND + d] = pp;
             }
+        }
+    }
+    // x0 -> x0 + delta e_comp for the orbit (neighbouring initial conditions); comp in the
+    // ordering of y.  psign is the momentum sign load() applied: the displacement is of the ORIGINAL IC.
+    __device__ __forceinline__ void displace(int comp, double delta, double psign) {
+        if (lt != 0) return;
+#pragma unroll
+        for (int d = 0; d < ND; d++) {
+            if (comp == d) q[d] += delta;
+            if (comp == ND + d) p[d] += psign * delta;
         }
     }
     __device__ __forceinline__ void store(double* y, double* w, long long n_ic, long long ic, bool bad) const {
@@ -773,15 +787,20 @@ ld_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const R
           int n_dirs) {
     constexpr int NI = C::NI, L = C::L;
     const long long gt = (long long)blockIdx.x * TPB + threadIdx.x;
-    const long long task = gt / L, n_task = a.n_ic * n_dirs;
+    const long long per_dir = a.n_ic * a.n_members;  // tasks are ordered [direction][member][ic]
+    const long long task = gt / L, n_task = per_dir * n_dirs;
     const bool valid = task < n_task;
     if (L == 1 && !valid) return;
     const long long tk = valid ? task : n_task - 1;  // padding tiles shadow the last task (shuffles stay convergent)
-    const int dsel = dir_first + (int)(tk / a.n_ic);  // 0 forward, 1 backward
-    const long long ic = tk % a.n_ic;
+    const int dsel = dir_first + (int)(tk / per_dir);  // 0 forward, 1 backward
+    const long long slot = tk % per_dir;                // = member * n_ic + ic: the output index
+    const int member = (int)(slot / a.n_ic);
+    const long long ic = slot % a.n_ic;
+    const double psign = dsel == 0 ? 1.0 : -1.0;
     C s;
     s.init(prm);
-    s.load(a.y0, nullptr, a.n_ic, ic, dsel == 0 ? 1.0 : -1.0);
+    s.load(a.y0, nullptr, a.n_ic, ic, psign);
+    if (member > 0) s.displace((member - 1) >> 1, ((member - 1) & 1) ? -a.sigma : a.sigma, psign);
     double M = 0.0;
     const ForceFn<C> force{s};
     LdHook<C> hook{tab, s, M};
@@ -799,7 +818,7 @@ ld_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const R
     }
     const bool ok = s.finite_all();
     double* out = dsel == 0 ? a.ld_fwd : a.ld_bwd;
-    if (valid && s.lt == 0) out[ic] = ok ? M : nan("");
+    if (valid && s.lt == 0) out[slot] = ok ? M : nan("");
 }
 
 }  // namespace chs

@@ -37,7 +37,7 @@ int run_chain_ld_t(const LaunchReq& rq) {
     if (!fput_params(rq, prm)) return (int)cudaErrorInvalidValue;
     if (rq.fput_n > LT * PPL || (!PAD && rq.fput_n != LT * PPL)) return (int)cudaErrorInvalidValue;
     auto kern = ld_kernel<Chain<LT, PPL, 0, PAD>, TPB, MINB>;
-    const long long n_threads = rq.args.n_ic * rq.n_dirs * LT;
+    const long long n_threads = rq.args.n_ic * rq.args.n_members * rq.n_dirs * LT;
     int r = finish_launch(rq, kern, TPB, LT, n_threads);
     if (r != -2) return r;
     const long long blocks = (n_threads + TPB - 1) / TPB;

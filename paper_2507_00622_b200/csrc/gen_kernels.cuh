@@ -247,13 +247,20 @@ gen_ld_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, c
               int n_dirs) {
     constexpr int N = Sys::N;
     const long long gt = (long long)blockIdx.x * TPB + threadIdx.x;
-    if (gt >= a.n_ic * n_dirs) return;
-    const int dsel = dir_first + (int)(gt / a.n_ic);
-    const long long ic = gt % a.n_ic;
+    const long long per_dir = a.n_ic * a.n_members;  // tasks are ordered [direction][member][ic]
+    if (gt >= per_dir * n_dirs) return;
+    const int dsel = dir_first + (int)(gt / per_dir);
+    const long long slot = gt % per_dir;
+    const int member = (int)(slot / a.n_ic);
+    const long long ic = slot % a.n_ic;
     const double psign = dsel == 0 ? 1.0 : -1.0;
     double y[N];
 #pragma unroll
-    for (int c = 0; c < N; c++) y[c] = a.y0[(long long)c * a.n_ic + ic] * (c >= N / 2 ? psign : 1.0);
+    for (int c = 0; c < N; c++) {
+        double v = a.y0[(long long)c * a.n_ic + ic];
+        if (member > 0 && c == ((member - 1) >> 1)) v += ((member - 1) & 1) ? -a.sigma : a.sigma;  // neighbour
+        y[c] = v * (c >= N / 2 ? psign : 1.0);
+    }
     double M = 0.0;
     for (long long st = 0; st < a.n_steps; ++st) {
         double K[12][N];
@@ -281,7 +288,7 @@ gen_ld_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, c
 #pragma unroll
     for (int c = 0; c < N; c++) ok = ok && isfinite(y[c]);
     double* out = dsel == 0 ? a.ld_fwd : a.ld_bwd;
-    out[ic] = ok ? M : nan("");
+    out[slot] = ok ? M : nan("");
 }
 
 }  // namespace chs

@@ -22,7 +22,7 @@ int run_gen_ld(const LaunchReq& rq) {
     typename Sys::Params prm;
     if (!Sys::make_params(rq.params, rq.n_params, prm)) return (int)cudaErrorInvalidValue;
     auto kern = gen_ld_kernel<Sys, TPB, MINB>;
-    const long long n_threads = rq.args.n_ic * rq.n_dirs;
+    const long long n_threads = rq.args.n_ic * rq.args.n_members * rq.n_dirs;
     int r = finish_launch(rq, kern, TPB, 1, n_threads);
     if (r != -2) return r;
     const long long blocks = (n_threads + TPB - 1) / TPB;

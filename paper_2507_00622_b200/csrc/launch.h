@@ -107,7 +107,7 @@ inline int run_ld(const LaunchReq& rq) {
     typename Sys::Params prm;
     if (!Sys::make_params(rq.params, rq.n_params, prm)) return (int)cudaErrorInvalidValue;
     auto kern = ld_kernel<Col<Sys, 0, 1>, TPB, MINB>;
-    const long long n_threads = rq.args.n_ic * rq.n_dirs;
+    const long long n_threads = rq.args.n_ic * rq.args.n_members * rq.n_dirs;
     int r = finish_launch(rq, kern, TPB, 1, n_threads);
     if (r != -2) return r;
     const long long blocks = (n_threads + TPB - 1) / TPB;

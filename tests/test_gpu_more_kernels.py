@@ -396,3 +396,53 @@ def test_zero_length_runs(chs, orc):
         assert (rep.n_accepted.cpu().numpy() == 0).all() and (rep.status.cpu().numpy() == 0).all()
         lam = chs.lyap(HH, None, dev(y0), dev(w0), renorm_every=1, **kw).cpu().numpy()
         assert np.isnan(lam).all()
+
+
+# ---------------------------------------------------------------------------- LD neighbours
+@pytest.mark.parametrize("case", ["hh", "coupled3", "fput12", "fput100", "dp"])
+def test_ld_neighbours(chs, orc, case):
+    """the 2n axis neighbours x0 +- sigma e_i of every IC are generated on the device and
+    integrated in the same LD launch as the centres; members' LDs element-wise against the oracle's plain
+    loop over displaced ICs, raw differences |M(x0 +- sigma e_i) - M(x0)| to an absolute 1e-9 M."""
+    if case == "hh":
+        sysid, prm, y0, h, ns, sg = HH, None, W.hh_grid(0.125, 19, 7), 0.01, 1500, 1e-3     # 133 ICs, ragged
+    elif case == "coupled3":
+        sysid, prm, y0, h, ns, sg = C3, W.coupled3_params(0.1), W.coupled3_ics(70, seed=1), 0.01, 1000, 1e-2
+    elif case == "fput12":     # padded in-warp tile: members displace particles of a 12-chain on a 16-slot tile
+        sysid, prm, y0, h, ns, sg = FPUT, W.fput_params(12, 1.0, 0.1, 0.8), W.fput_ics(9, 12, seed=5, E=1.2), 0.05, 400, 1e-3
+    elif case == "fput100":    # wide tile (one block per member)
+        sysid, prm, y0, h, ns, sg = FPUT, W.fput_params(100, 1.0, 0.0, 1.0), W.fput_ics(2, 100, seed=6, E=10.0), 0.05, 200, 1e-3
+    else:
+        sysid, prm, y0, h, ns, sg = W.SYS_DOUBLE_PENDULUM, (1.0, 1.0), W.double_pendulum_ics(50, seed=3), 0.01, 800, 1e-3
+    n, n_ic = y0.shape
+    ro = orc.ld_neighbours(sysid, prm, y0, sg, 0.0, h, ns, precision="f80")
+    rg = chs.ld_neighbours(sysid, prm, dev(y0), sg, 0.0, h, ns)
+    for key in ("fwd", "bwd"):
+        g, o = rg[key].cpu().numpy(), ro[key]
+        assert g.shape == o.shape == (1 + 2 * n, n_ic)
+        assert np.abs(g / o - 1).max() <= 1e-8, key
+    for key, ctr in (("diff_fwd", "fwd"), ("diff_bwd", "bwd")):
+        g, o = rg[key].cpu().numpy(), ro[key]
+        assert g.shape == (2 * n, n_ic) and np.abs(g - o).max() <= 1e-9 * ro[ctr][0].max(), key
+        assert o.max() > 0.0
+    # the centre row is chaoticus_ld itself, bit for bit; one direction only; no differences
+    f, b = chs.ld(sysid, prm, dev(y0), 0.0, h, ns)
+    assert (rg["fwd"][0] == f).all().item() and (rg["bwd"][0] == b).all().item()
+    r1 = chs.ld_neighbours(sysid, prm, dev(y0), sg, 0.0, h, ns, backward=False, diffs=False)
+    assert r1["bwd"] is None and r1["diff_fwd"] is None and (r1["fwd"] == rg["fwd"]).all().item()
+
+
+def test_ld_neighbours_host_and_errors(chs):
+    import torch
+    y0 = W.hh_grid(0.125, 6, 5)
+    rg = chs.ld_neighbours(HH, None, dev(y0), 2e-3, 0.0, 0.01, 300)
+    f, b, df, db = np.empty((9, 30)), np.empty((9, 30)), np.empty((8, 30)), np.empty((8, 30))
+    chs.ld_neighbours_host(HH, None, y0, 2e-3, 0.0, 0.01, 300, f, b, df, db)
+    assert (rg["fwd"].cpu().numpy() == f).all() and (rg["bwd"].cpu().numpy() == b).all()
+    assert (rg["diff_fwd"].cpu().numpy() == df).all() and (rg["diff_bwd"].cpu().numpy() == db).all()
+    z = chs.ld_neighbours(HH, None, dev(y0), 0.0, 0.0, 0.01, 300)       # sigma = 0: every member is the centre
+    assert (z["fwd"] == z["fwd"][0]).all().item() and (z["diff_fwd"] == 0).all().item()
+    with pytest.raises(chs.ChaoticusError):
+        chs.ld_neighbours(HH, None, dev(y0), -1.0, 0.0, 0.01, 10)
+    e = torch.empty((4, 0), dtype=torch.float64, device="cuda")
+    assert chs.ld_neighbours(HH, None, e, 1e-3, 0.0, 0.01, 10)["fwd"].shape == (9, 0)
