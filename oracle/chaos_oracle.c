@@ -61,7 +61,7 @@ typedef double real;
 #define SYS_HENON_HEILES 0
 #define SYS_COUPLED3 1
 #define SYS_FPUT 2
-#define SYS_DOUBLE_PENDULUM 3 /* orbit only (no variational equations): PAPER.md:66-81 */
+#define SYS_DOUBLE_PENDULUM 3 /* PAPER.md:66-81, not separable */
 
 /* per-trajectory status words */
 #define ST_OK 0
@@ -215,8 +215,7 @@ static real fput_energy(const double *P, const real *y)
  *   theta' = B^-1(x) p,  x = cos(theta1 - theta2)
  *   p'     = sin(Dtheta)/2 * (p^T C(x) p) * (1, -1)^T - (alpha (1+sigma) sin theta1, sin theta2)^T
  *   C(x)   = -B^-1 (dB/dx) B^-1, formed here by the two matrix products,
- * with B the inverse of Eq.(2): B = [[alpha^2 (1+sigma), alpha x],[alpha x, 1]], dB/dx = [[0,alpha],[alpha,0]].
- * Orbit only: the paper prints no variational equations for this system. */
+ * with B the inverse of Eq.(2): B = [[alpha^2 (1+sigma), alpha x],[alpha x, 1]], dB/dx = [[0,alpha],[alpha,0]]. */
 static void dp_binv(real sg, real al, real x, real Bi[2][2])
 {
     real den = 1 + sg - x * x;
@@ -245,6 +244,55 @@ static void dp_orbit(const double *P, const real *y, real *f)
     f[1] = Bi[1][0] * p1 + Bi[1][1] * p2;
     f[2] = sd / 2 * pCp - al * (1 + sg) * s1;
     f[3] = -(sd / 2 * pCp) - s2;
+}
+/* Variational equations of Eq.(3) (deviation vectors "satisfy the variational equations of
+ * the system"; the paper does not print them for this system): the derivative of the right-hand side above
+ * along w = (dth1, dth2, dp1, dp2), term by term, with x = cos(Dtheta), s = sin(Dtheta), dD = dth1 - dth2,
+ * dx = -s dD:
+ *   d(theta')  = B^-1 dp + dx C p
+ *   d(p'_1)    = dS - alpha (1+sigma) cos(theta1) dth1,   d(p'_2) = -dS - cos(theta2) dth2,
+ *   S = (s/2) p^T C p,   dS = (x/2) dD p^T C p + (s/2) [2 p^T C dp + dx p^T C' p],
+ *   C' = dC/dx = -(C B' B^-1 + B^-1 B' C)    (from C = -B^-1 B' B^-1 with B' = dB/dx constant),
+ * every matrix formed by the products as written. */
+static void mat2_mul(const real A[2][2], const real Bm[2][2], real Cm[2][2])
+{
+    for (int i = 0; i < 2; i++)
+        for (int j = 0; j < 2; j++) Cm[i][j] = A[i][0] * Bm[0][j] + A[i][1] * Bm[1][j];
+}
+static real quad2(const real A[2][2], const real *u, const real *v) /* u^T A v */
+{
+    return u[0] * (A[0][0] * v[0] + A[0][1] * v[1]) + u[1] * (A[1][0] * v[0] + A[1][1] * v[1]);
+}
+static void dp_dev(const double *P, const real *y, const real *w, real *g)
+{
+    real sg = P[0], al = P[1];
+    real th1 = y[0], th2 = y[1];
+    const real *p = y + 2, *dth = w, *dpv = w + 2;
+    real dth12 = th1 - th2;
+#ifdef ORC_REAL_IS_LONG_DOUBLE
+    real x = cosl(dth12), sn = sinl(dth12), c1 = cosl(th1), c2 = cosl(th2);
+#else
+    real x = cos(dth12), sn = sin(dth12), c1 = cos(th1), c2 = cos(th2);
+#endif
+    real Bi[2][2], dB[2][2] = {{0, al}, {al, 0}}, T[2][2], C[2][2], U[2][2], V[2][2], Cp[2][2];
+    dp_binv(sg, al, x, Bi);
+    mat2_mul(Bi, dB, T);
+    mat2_mul(T, Bi, C);
+    for (int i = 0; i < 2; i++)
+        for (int j = 0; j < 2; j++) C[i][j] = -C[i][j];          /* C  = -B^-1 B' B^-1 */
+    mat2_mul(C, dB, T);
+    mat2_mul(T, Bi, U);                                          /* C B' B^-1 */
+    mat2_mul(Bi, dB, T);
+    mat2_mul(T, C, V);                                           /* B^-1 B' C */
+    for (int i = 0; i < 2; i++)
+        for (int j = 0; j < 2; j++) Cp[i][j] = -(U[i][j] + V[i][j]); /* C' */
+    real dD = dth[0] - dth[1], dx = -sn * dD;
+    real pCp = quad2(C, p, p);
+    real dS = x / 2 * dD * pCp + sn / 2 * (2 * quad2(C, p, dpv) + dx * quad2(Cp, p, p));
+    g[0] = Bi[0][0] * dpv[0] + Bi[0][1] * dpv[1] + dx * (C[0][0] * p[0] + C[0][1] * p[1]);
+    g[1] = Bi[1][0] * dpv[0] + Bi[1][1] * dpv[1] + dx * (C[1][0] * p[0] + C[1][1] * p[1]);
+    g[2] = dS - al * (1 + sg) * c1 * dth[0];
+    g[3] = -dS - c2 * dth[1];
 }
 static real dp_energy(const double *P, const real *y)
 {
@@ -279,7 +327,8 @@ static void rhs_aug(const prob_t *pb, const real *Y, real *F)
         for (int v = 1; v <= pb->k; v++) fput_dev(pb->params, Y, Y + v * n, F + v * n);
         break;
     case SYS_DOUBLE_PENDULUM:
-        dp_orbit(pb->params, Y, F); /* k = 0 only (checked by the entry points) */
+        dp_orbit(pb->params, Y, F);
+        for (int v = 1; v <= pb->k; v++) dp_dev(pb->params, Y, Y + v * n, F + v * n);
         break;
     }
 }
@@ -675,7 +724,6 @@ int orc_run(int sys, const double *params, long long n_ic, double *y, double *w,
 {
     int n = orc_dim(sys, params);
     if (n < 0 || n_ic < 0 || k < 0 || (k > 0 && !w) || !y) return ORC_EINVAL;
-    if (sys == SYS_DOUBLE_PENDULUM && k > 0) return ORC_EINVAL; /* orbit only */
     if (mode != MODE_NONE && (k < 1 || renorm_every < 1)) return ORC_EINVAL;
     if (indicator == IND_SALI && k != 2) return ORC_EINVAL;
     if (indicator == IND_GALI && (k < 2 || k > n)) return ORC_EINVAL;
