@@ -39,7 +39,7 @@ extern "C" {
 
 typedef enum { CHS_OK = 0, CHS_EINVAL = 1, CHS_EUNSUPPORTED = 2, CHS_ECUDA = 3 } chs_rc;
 
-/* Systems (all separable, H = |p|^2/2 + V(q)):
+/* Systems (the first three separable, H = |p|^2/2 + V(q)):
  *  CHS_SYS_HENON_HEILES  n = 4, no params.  PAPER.md:87 Eq.(4), Eq.(5).
  *  CHS_SYS_COUPLED3      n = 6, params (omega1, omega2, omega3, eps):
  *                        V = sum omega_i^2 q_i^2 / 2 + eps q1^2 q2 + eps q2^2 q3
@@ -50,9 +50,9 @@ typedef enum { CHS_OK = 0, CHS_EINVAL = 1, CHS_EUNSUPPORTED = 2, CHS_ECUDA = 3 }
  *                        (integration, LD, SALI, GALI_4, Lyapunov k = 4; N = 8 also GALI_2,3 and k = 1,2).
  *  CHS_SYS_DOUBLE_PENDULUM  n = 4, params (sigma, alpha) = (mass ratio, length ratio); state
  *                        (theta1, theta2, p1, p2).  NOT separable: Eq.(1)
- *                        Eq.(2), Eq.(3).  Orbit only: chaoticus_integrate_fixed /
- *                        _adaptive and chaoticus_ld (generic first-order kernel); the entry points
- *                        that need variational equations return CHS_EUNSUPPORTED for it. */
+ *                        Eq.(2), Eq.(3); generic first-order kernels.  Integration (fixed,
+ *                        adaptive), LD, SALI (fixed, adaptive), GALI_2..4, Lyapunov k = 1, 2, 4 (k = 1, 4
+ *                        also adaptive); variational equations = the derivative of Eq.(3). */
 typedef enum { CHS_SYS_HENON_HEILES = 0, CHS_SYS_COUPLED3 = 1, CHS_SYS_FPUT = 2, CHS_SYS_DOUBLE_PENDULUM = 3 } chs_system;
 
 typedef struct {

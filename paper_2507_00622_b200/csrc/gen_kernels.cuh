@@ -3,8 +3,9 @@
 // The dimensionless double pendulum (Eq.(1)-(3)) has a kinetic energy that depends
 // on the angles, so the separable rearrangement of dop8_core.cuh does not apply: here the method
 // runs in its textbook form, y' = f(y), 12 full stage derivative vectors K_i (n = 4 components:
-// 9 live stage vectors = 36 doubles, fits registers), one trajectory per thread.  Orbit only
-// (the paper prints no variational equations for this system).  Fixed step: tableau premultiplied
+// 9 live stage vectors = 36 doubles, fits registers), one trajectory per thread for the orbit alone
+// (gen_run_kernel, gen_ld_kernel) and a tile of lanes, one column per lane, when deviation vectors ride
+// along (gen_col_kernel).  Fixed step: tableau premultiplied
 // by h in the constant bank; adaptive: raw tableau, per-trajectory h, the same controller as
 // run_kernel.
 #pragma once
@@ -36,6 +37,60 @@ struct DoublePendulum {
         const double t = 0.5 * sd * pCp;
         f[2] = fma(-P.asg, s1, t);
         f[3] = -t - s2;
+    }
+    // ---- variational equations: the derivative of Eq.(3) along w = (dth1, dth2, dp1, dp2).
+    // Everything that depends on the orbit's stage state only is formed once per stage (Lin), then a
+    // deviation column costs ~25 FP64 instructions.  With id = 1/D, M' = dM/dx = [[0, -1/alpha], [-1/alpha, 0]]:
+    //   B^-1 = M id,  C = 2x M id^2 + M' id,  C' = dC/dx = (2M + 4x M') id^2 + 8 x^2 M id^3
+    //   d(theta') = B^-1 dp + dx C p,  dx = -sin(Dtheta) (dth1 - dth2)
+    //   dS = (x/2) dD p^T C p + (s/2) [2 (C p)^T dp + dx p^T C' p]
+    //   d(p1') = dS - alpha (1+sigma) cos(theta1) dth1,   d(p2') = -dS - cos(theta2) dth2
+    // (the oracle forms C and C' by matrix products of B^-1 and dB/dx instead).
+    static constexpr int NDOF = 2;
+    struct Hess {};  // Col<DoublePendulum, K, L> only stores the state; its separable force() is never used
+    struct Pre {};
+    struct Lin {
+        double b00, b01, b11, u0, u1, hx_pCp, hs, hs_pCpp, sn, a1c1, c2;
+        double f[4];  // the orbit's own right-hand side at the same state
+    };
+    __device__ static __forceinline__ Lin lin(const Params& P, const double (&y)[4]) {
+        double s1, c1, s2, c2;
+        sincos(y[0], &s1, &c1);
+        sincos(y[1], &s2, &c2);
+        const double x = fma(c1, c2, s1 * s2), sd = fma(s1, c2, -c1 * s2);
+        const double p1 = y[2], p2 = y[3];
+        const double id = 1.0 / fma(-x, x, P.sg1), id2 = id * id;
+        const double m01 = -x * P.ia;
+        const double Mp0 = fma(P.ia2, p1, m01 * p2), Mp1 = fma(m01, p1, P.sg1 * p2);  // M p
+        const double pMp = fma(p1, Mp0, p2 * Mp1), pM1p = -2.0 * P.ia * p1 * p2;           // p^T M p, p^T M' p
+        const double pCp = fma(2.0 * x * id2, pMp, id * pM1p);
+        const double pCpp = fma(id2, fma(4.0 * x, pM1p, 2.0 * pMp), 8.0 * x * x * id2 * id * pMp);
+        Lin L;
+        L.b00 = P.ia2 * id;
+        L.b01 = m01 * id;
+        L.b11 = P.sg1 * id;
+        L.u0 = fma(2.0 * x * id2, Mp0, -P.ia * id * p2);  // C p
+        L.u1 = fma(2.0 * x * id2, Mp1, -P.ia * id * p1);
+        L.hx_pCp = 0.5 * x * pCp;
+        L.hs = 0.5 * sd;
+        L.hs_pCpp = 0.5 * sd * pCpp;
+        L.sn = sd;
+        L.a1c1 = P.asg * c1;
+        L.c2 = c2;
+        const double t = 0.5 * sd * pCp;
+        L.f[0] = id * Mp0;
+        L.f[1] = id * Mp1;
+        L.f[2] = fma(-P.asg, s1, t);
+        L.f[3] = -t - s2;
+        return L;
+    }
+    __device__ static __forceinline__ void apply_lin(const Lin& L, const double (&w)[4], double (&g)[4]) {
+        const double dD = w[0] - w[1], dx = -L.sn * dD;
+        g[0] = fma(L.b00, w[2], fma(L.b01, w[3], dx * L.u0));
+        g[1] = fma(L.b01, w[2], fma(L.b11, w[3], dx * L.u1));
+        const double dS = fma(L.hx_pCp, dD, fma(2.0 * L.hs, fma(L.u0, w[2], L.u1 * w[3]), dx * L.hs_pCpp));
+        g[2] = fma(-L.a1c1, w[0], dS);
+        g[3] = fma(-L.c2, w[1], -dS);
     }
     __host__ static bool make_params(const double* p, int n, Params& out) {
         if (n < 2 || !(p[1] > 0.0) || !(p[0] > -1.0)) return false;
@@ -289,6 +344,283 @@ gen_ld_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, c
     for (int c = 0; c < N; c++) ok = ok && isfinite(y[c]);
     double* out = dsel == 0 ? a.ld_fwd : a.ld_bwd;
     out[slot] = ok ? M : nan("");
+}
+
+// ---- generic form WITH deviation vectors: one column per lane ------------------------------------
+// PAPER.md:49-52 (solvers 3-6) for a non-separable system.  A trajectory is a tile of L >= 1 + K lanes:
+// lane 0 the orbit, lane v deviation vector v, each lane its 4 components and 12 full stage derivatives in
+// registers (the whole augmented state on one thread would need > 255 registers at K = 2).  Per stage the
+// orbit's stage state is broadcast from lane 0 (4 shuffles), every lane forms the orbit-only terms (the two
+// sincos, B^-1, C p, p^T C p, p^T C' p) and then takes f(Y) (lane 0) or Df(Y) w (the others).  State,
+// renormalisation, Gram-Schmidt, SALI / GALI and the stores are the column layout's (Col<Sys, K, L>).
+template <class Sys, int K, int L, int MODE, int IND, bool ADAPT, int TPB, int MINB>
+__global__ void __launch_bounds__(TPB, MINB)
+gen_col_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, const RunArgs a) {
+    using C = Col<Sys, K, L>;
+    static_assert(C::CPL == 1 && C::ND == 2 && Sys::N == 4, "one column of 4 components per lane");
+    constexpr int N = 4;
+    const long long gt = (long long)blockIdx.x * TPB + threadIdx.x;
+    const long long traj = gt / L;
+    const bool valid = traj < a.n_ic;
+    const long long ic = valid ? traj : a.n_ic - 1;  // padding tiles shadow the last trajectory
+    const bool want_log = (a.logacc != nullptr) || (a.lambda != nullptr);
+    C s;
+    s.init(prm);
+    s.load(a.y, a.w, a.n_ic, ic, 1.0);
+    double qc[2] = {0.0, 0.0}, pc[2] = {0.0, 0.0};  // carried rounding words (orbit lane), as run_kernel
+    if (a.resume) {
+        if (a.carry && !ADAPT) s.load_carry(a.carry, a.n_ic, ic, qc, pc);
+    } else {
+        s.template do_renorm<MODE>(false, true);
+    }
+    long long n_acc = 0, n_rej = 0;
+    int status = ST_OK;
+    double t = a.t0;
+    const bool orbit = (s.lt == 0);
+
+    // stage derivatives of one step of size h from (s.q, s.p); PREMUL as dop8_generic_stages
+    auto stages = [&](auto premul, double h, double (&Kd)[12][N]) {
+        constexpr bool PREMUL = decltype(premul)::value;
+        const double y[N] = {s.q[0], s.q[1], s.p[0], s.p[1]};
+        static_for<0, 12>([&](auto icn) {
+            constexpr int i = decltype(icn)::value;
+            double Y[N];
+#pragma unroll
+            for (int c = 0; c < N; c++) {
+                if constexpr (i == 0) {
+                    Y[c] = y[c];
+                } else if constexpr (PREMUL) {
+                    double acc = y[c];
+                    static_for<0, i>([&](auto jc) {
+                        constexpr int j = decltype(jc)::value;
+                        if constexpr (coef::A[i][j] != 0.0) acc = fma(tab.ap[i][j], Kd[j][c], acc);
+                    });
+                    Y[c] = acc;
+                } else {
+                    double sm = tab.ap[i][0] * Kd[0][c];
+                    static_for<1, i>([&](auto jc) {
+                        constexpr int j = decltype(jc)::value;
+                        if constexpr (coef::A[i][j] != 0.0) sm = fma(tab.ap[i][j], Kd[j][c], sm);
+                    });
+                    Y[c] = fma(h, sm, y[c]);
+                }
+            }
+            double Yo[N];
+#pragma unroll
+            for (int c = 0; c < N; c++) Yo[c] = tile_bcast<L>(Y[c], 0);
+            const typename Sys::Lin ln = Sys::lin(prm, Yo);
+            double g[N];
+            Sys::apply_lin(ln, Y, g);
+#pragma unroll
+            for (int c = 0; c < N; c++) Kd[i][c] = orbit ? ln.f[c] : g[c];
+        });
+    };
+    // y+ = y + (inc + carried word), Fast2Sum; returns the new carried words
+    auto advance = [&](const double (&inc)[N], double (&yn)[N], double (&ycn)[N]) {
+        const double y[N] = {s.q[0], s.q[1], s.p[0], s.p[1]};
+        const double yc[N] = {qc[0], qc[1], pc[0], pc[1]};
+#pragma unroll
+        for (int c = 0; c < N; c++) {
+            const double u = inc[c] + yc[c];
+            const double sm = y[c] + u;
+            ycn[c] = u - (sm - y[c]);
+            yn[c] = sm;
+        }
+    };
+    auto commit = [&](const double (&yn)[N], const double (&ycn)[N]) {
+        s.q[0] = yn[0]; s.q[1] = yn[1]; s.p[0] = yn[2]; s.p[1] = yn[3];
+        qc[0] = ycn[0]; qc[1] = ycn[1]; pc[0] = ycn[2]; pc[1] = ycn[3];
+    };
+
+    long long slot = 0;
+    if constexpr (!ADAPT) {
+        int cd = a.m, sd = a.sample_every;
+        for (long long st = 1; st <= a.n_steps; ++st) {
+            double Kd[12][N];
+            stages(std::true_type{}, 0.0, Kd);
+            double inc[N], yn[N], ycn[N];
+#pragma unroll
+            for (int c = 0; c < N; c++) {
+                double sm = tab.bp[0] * Kd[0][c];
+                static_for<1, 12>([&](auto lc) {
+                    constexpr int l = decltype(lc)::value;
+                    if constexpr (coef::B[l] != 0.0) sm = fma(tab.bp[l], Kd[l][c], sm);
+                });
+                inc[c] = sm;
+            }
+            advance(inc, yn, ycn);
+            commit(yn, ycn);
+            if constexpr (MODE != MODE_NONE) {
+                if (--cd == 0 || st == a.n_steps) {
+                    cd = a.m;
+                    s.template do_renorm<MODE>(want_log, true);
+                    s.scrub_carry(qc, pc);
+                    if constexpr (IND != IND_NONE) {
+                        if (a.sample_every > 0 && --sd == 0) {
+                            sd = a.sample_every;
+                            if (slot < a.n_samples - 1) {
+                                const double v = s.template indicator<IND>();
+                                if (valid && s.lt == 0) a.series[slot * a.n_ic + ic] = v;
+                                slot++;
+                            }
+                        }
+                    }
+                }
+            }
+        }
+        n_acc = a.n_steps;
+        t = a.t0 + (double)a.n_steps * a.h;
+    } else {
+        // adaptive: the tile's decisions come from tile-wide sums, identical on
+        // all its lanes; tiles of one warp differ, so the loop is warp-uniform and commits are predicated
+        const double dir = (a.t_end >= a.t0) ? 1.0 : -1.0;
+        const double interval = fabs(a.t_end - a.t0);
+        constexpr double D = (double)(N * (1 + K));
+        const bool on = s.lt <= K;
+        double h_abs = a.h0;
+        if (!(h_abs > 0.0)) {  // starting step, item 6
+            h_abs = 0.0;
+            if (interval > 0.0) {
+                const double y[N] = {s.q[0], s.q[1], s.p[0], s.p[1]};
+                double Yo[N], f0[N], f1[N], y1[N], g[N];
+#pragma unroll
+                for (int c = 0; c < N; c++) Yo[c] = tile_bcast<L>(y[c], 0);
+                typename Sys::Lin ln = Sys::lin(prm, Yo);
+                Sys::apply_lin(ln, y, g);
+                double s0 = 0.0, s1 = 0.0, s2 = 0.0;
+#pragma unroll
+                for (int c = 0; c < N; c++) {
+                    f0[c] = orbit ? ln.f[c] : g[c];
+                    const double is = 1.0 / fma(fabs(y[c]), a.rtol, a.atol);
+                    if (on) {
+                        s0 += (y[c] * is) * (y[c] * is);
+                        s1 += (f0[c] * is) * (f0[c] * is);
+                    }
+                }
+                const double d0 = sqrt(tile_sum<L>(s0) / D), d1 = sqrt(tile_sum<L>(s1) / D);
+                double ha = (d0 < 1e-5 || d1 < 1e-5) ? 1e-6 : 0.01 * d0 / d1;
+                ha = fmin(ha, interval);
+#pragma unroll
+                for (int c = 0; c < N; c++) y1[c] = fma(ha * dir, f0[c], y[c]);
+#pragma unroll
+                for (int c = 0; c < N; c++) Yo[c] = tile_bcast<L>(y1[c], 0);
+                ln = Sys::lin(prm, Yo);
+                Sys::apply_lin(ln, y1, g);
+#pragma unroll
+                for (int c = 0; c < N; c++) {
+                    f1[c] = orbit ? ln.f[c] : g[c];
+                    const double is = 1.0 / fma(fabs(y[c]), a.rtol, a.atol);
+                    const double d = (f1[c] - f0[c]) * is;
+                    if (on) s2 += d * d;
+                }
+                const double d2 = sqrt(tile_sum<L>(s2) / D) / ha;
+                const double hb = (d1 <= 1e-15 && d2 <= 1e-15) ? fmax(1e-6, 1e-3 * ha) : root8(0.01 / fmax(d1, d2));
+                h_abs = fmin(fmin(100.0 * ha, hb), interval);
+            }
+        }
+        long long attempts = 0;
+        bool rejected = false;
+        double min_step = 0.0;
+        int cd = a.m;
+        while (true) {
+            bool active = status == ST_OK && dir * (a.t_end - t) > 0.0;
+            if (!__any_sync(0xffffffffu, active)) break;
+            if (!rejected) {
+                min_step = 10.0 * fabs(nextafter(t, dir * INFINITY) - t);
+                h_abs = fmax(h_abs, min_step);
+            }
+            if (active && h_abs < min_step) { status = ST_UNDERFLOW; active = false; }
+            if (active && a.max_steps > 0 && attempts >= a.max_steps) { status = ST_MAXSTEPS; active = false; }
+            attempts += active ? 1 : 0;
+            double t_new = t + h_abs * dir;
+            if (dir * (t_new - a.t_end) > 0.0) t_new = a.t_end;
+            const double h = t_new - t, h_try = fabs(h);
+            double Kd[12][N];
+            stages(std::false_type{}, h, Kd);
+            double inc[N], yn[N], ycn[N], e5[N], e3[N];
+#pragma unroll
+            for (int c = 0; c < N; c++) {
+                double sm = tab.bp[0] * Kd[0][c], a5 = tab.e5p[0] * Kd[0][c], a3 = tab.e3p[0] * Kd[0][c];
+                static_for<1, 12>([&](auto lc) {
+                    constexpr int l = decltype(lc)::value;
+                    if constexpr (coef::B[l] != 0.0) sm = fma(tab.bp[l], Kd[l][c], sm);
+                    if constexpr (coef::E5[l] != 0.0) a5 = fma(tab.e5p[l], Kd[l][c], a5);
+                    if constexpr (coef::E3[l] != 0.0) a3 = fma(tab.e3p[l], Kd[l][c], a3);
+                });
+                inc[c] = h * sm;
+                e5[c] = a5;
+                e3[c] = a3;
+            }
+            advance(inc, yn, ycn);
+            double S5 = 0.0, S3 = 0.0;
+            {
+                const double y[N] = {s.q[0], s.q[1], s.p[0], s.p[1]};
+#pragma unroll
+                for (int c = 0; c < N; c++) {
+                    const double is = fast_rcp(fma(a.rtol, fmax(fabs(y[c]), fabs(yn[c])), a.atol));
+                    const double u = e5[c] * is, v = e3[c] * is;
+                    if (on) {
+                        S5 = fma(u, u, S5);
+                        S3 = fma(v, v, S3);
+                    }
+                }
+            }
+            S5 = tile_sum<L>(S5);
+            S3 = tile_sum<L>(S3);
+            const double err = (S5 == 0.0 && S3 == 0.0) ? 0.0 : h_try * S5 * fast_rsqrt((S5 + 0.01 * S3) * D);
+            bool ren = false;
+            if (active) {
+                if (err < 1.0) {
+                    double factor = (err == 0.0) ? 10.0 : fmin(10.0, 0.9 * inv_root8(err));
+                    if (rejected) factor = fmin(factor, 1.0);
+                    h_abs = h_try * factor;
+                    t = t_new;
+                    commit(yn, ycn);
+                    n_acc++;
+                    rejected = false;
+                    const bool at_end = !(dir * (a.t_end - t) > 0.0);
+                    if (MODE != MODE_NONE && (--cd == 0 || at_end)) {
+                        cd = a.m;
+                        ren = true;
+                    }
+                } else if (err >= 1.0) {
+                    h_abs = h_try * fmax(0.2, 0.9 * inv_root8(err));
+                    rejected = true;
+                    n_rej++;
+                } else {
+                    status = ST_NONFINITE;
+                }
+            }
+            if constexpr (MODE != MODE_NONE) {
+                if (__any_sync(0xffffffffu, ren)) {
+                    s.template do_renorm<MODE>(want_log, ren);
+                    if (ren) s.scrub_carry(qc, pc);
+                }
+            }
+        }
+    }
+    bool bad = !s.finite_all();
+    bad = tile_any<L>(status != ST_OK) || bad;
+    if (bad && status == ST_OK) status = ST_NONFINITE;
+    double ind = 0.0;
+    if constexpr (IND != IND_NONE) ind = s.template indicator<IND>();
+    if (!valid) return;
+    s.store(a.y, a.w, a.n_ic, ic, bad);
+    if (a.carry && !ADAPT) s.store_carry(a.carry, a.n_ic, ic, qc, pc, bad);
+    if constexpr (K > 0) s.store_logs(a, ic, bad, t - a.t0);
+    if (s.lt == 0) {
+        if constexpr (IND != IND_NONE) {
+            if (a.series) {
+                a.series[(a.n_samples - 1) * a.n_ic + ic] = bad ? nan("") : ind;
+                if (bad)
+                    for (long long r = slot; r < a.n_samples - 1; r++) a.series[r * a.n_ic + ic] = nan("");
+            }
+        }
+        if (a.n_acc) a.n_acc[ic] = n_acc;
+        if (a.n_rej) a.n_rej[ic] = n_rej;
+        if (a.status) a.status[ic] = status;
+        if (a.t_final) a.t_final[ic] = t;
+    }
 }
 
 }  // namespace chs

@@ -344,7 +344,7 @@ def test_double_pendulum_unsupported_entry_points(chs):
     y = dev(W.double_pendulum_ics(8))
     w = torch.zeros((2, 4, 8), dtype=torch.float64, device="cuda")
     with pytest.raises(chs.ChaoticusError, match="no compiled kernel"):
-        chs.sali(DP, (1.0, 1.0), y, w, h=0.01, n_steps=10)
+        chs.gali(DP, (1.0, 1.0), y, w, adaptive=True, t_end=1.0, rtol=1e-9, atol=1e-9)   # adaptive GALI: not compiled
     with pytest.raises(chs.ChaoticusError):
         chs.integrate_fixed(DP, (1.0, -1.0), y, 0.0, 0.01, 10)    # alpha <= 0
 
@@ -446,3 +446,87 @@ def test_ld_neighbours_host_and_errors(chs):
         chs.ld_neighbours(HH, None, dev(y0), -1.0, 0.0, 0.01, 10)
     e = torch.empty((4, 0), dtype=torch.float64, device="cuda")
     assert chs.ld_neighbours(HH, None, e, 1e-3, 0.0, 0.01, 10)["fwd"].shape == (9, 0)
+
+
+# ---------------------------------------------------------------------------- double pendulum, variational eqs
+def test_double_pendulum_sali_gali_lyap(chs, orc):
+    """Solvers 3-6 of PAPER.md:49-52 for the paper's first example system (non-separable, generic form,
+    one column per lane): states 1e-10, vectors 1e-9, indicators / exponents 1e-8 against the oracle."""
+    DP, prm = W.SYS_DOUBLE_PENDULUM, (1.0, 1.0)
+    n_ic = 75                                             # ragged: tiles of 2, 4, 8 lanes
+    y0 = W.double_pendulum_ics(n_ic, seed=3, theta_max=1.0, p_max=0.5)
+    w4 = W.deviation_vectors(n_ic, 4, 4, 41, "orthonormal")
+    w2 = np.ascontiguousarray(w4[:2])
+    # SALI, fixed step, sampled
+    yo, wo, lo = y0.copy(), w2.copy(), np.zeros((2, n_ic))
+    so = orc.sali(DP, prm, yo, wo, renorm_every=3, sample_every=50, lognorm=lo, h=0.01, n_steps=1500, precision="f80")["series"]
+    yg, wg, lg = dev(y0), dev(w2), dev(np.zeros((2, n_ic)))
+    sg = chs.sali(DP, prm, yg, wg, renorm_every=3, sample_every=50, lognorm=lg, h=0.01, n_steps=1500).cpu().numpy()
+    assert sg.shape == so.shape and so.min() > 1e-6
+    assert np.abs(sg / so - 1).max() <= 1e-8
+    assert rel_state(yg.cpu().numpy(), yo).max() <= 1e-10
+    assert np.abs(wg.cpu().numpy() - wo).max() <= 1e-9 and np.abs(lg.cpu().numpy() - lo).max() <= 1e-9
+    # GALI_k
+    for k in (2, 3, 4):
+        wk = np.ascontiguousarray(w4[:k])
+        go = orc.gali(DP, prm, y0.copy(), wk.copy(), renorm_every=5, sample_every=40, h=0.01, n_steps=1000, precision="f80")["series"]
+        gg = chs.gali(DP, prm, dev(y0), dev(wk), renorm_every=5, sample_every=40, h=0.01, n_steps=1000).cpu().numpy()
+        big = go > 1e-12
+        assert np.abs(gg[big] / go[big] - 1).max() <= 1e-8, k
+        assert np.abs(gg[~big] - go[~big]).max(initial=0.0) <= 1e-13, k
+    # Lyapunov k = 1, 2, 4 (full spectrum: sum = 0)
+    for k in (1, 2, 4):
+        wk = np.ascontiguousarray(w4[:k])
+        yo, wo = y0.copy(), wk.copy()
+        ro = orc.lyap(DP, prm, yo, wo, renorm_every=10, h=0.01, n_steps=2005, precision="f80")["lam"]
+        yg, wg = dev(y0), dev(wk)
+        lam = chs.lyap(DP, prm, yg, wg, renorm_every=10, h=0.01, n_steps=2005).cpu().numpy()
+        assert lam_err(lam, ro, 20.05) <= 1e-8, k
+        assert np.abs(wg.cpu().numpy() - wo).max() <= 1e-9
+        if k == 4:
+            assert np.abs(lam.sum(0)).max() <= 1e-11
+    # bit-identical continuation with the carried words
+    import torch
+    a_y, a_w, b_y, b_w = dev(y0), dev(w2), dev(y0), dev(w2)
+    sa = chs.sali(DP, prm, a_y, a_w, renorm_every=5, h=0.01, n_steps=600)
+    rep = chs.Report(n_ic, "cuda", n=4)
+    chs.sali(DP, prm, b_y, b_w, renorm_every=5, h=0.01, n_steps=250, report=rep)
+    rep.resume = True
+    sb = chs.sali(DP, prm, b_y, b_w, renorm_every=5, t0=2.5, h=0.01, n_steps=350, report=rep)
+    assert torch.equal(a_y, b_y) and torch.equal(a_w, b_w) and torch.equal(sa, sb)
+
+
+def test_double_pendulum_adaptive_and_classification(chs, orc):
+    DP, prm = W.SYS_DOUBLE_PENDULUM, (1.0, 1.0)
+    n_ic = 60
+    y0 = W.double_pendulum_ics(n_ic, seed=4, theta_max=1.0, p_max=0.5)
+    w4 = W.deviation_vectors(n_ic, 4, 4, 43, "orthonormal")
+    w2 = np.ascontiguousarray(w4[:2])
+    st = dict(adaptive=True, t_end=30.0, rtol=1e-11, atol=1e-11)
+    yo, wo = y0.copy(), w2.copy()
+    ro = orc.sali(DP, prm, yo, wo, renorm_every=2, precision="f80", **st)
+    yg, wg, rep = dev(y0), dev(w2), chs.Report(n_ic, "cuda")
+    sg = chs.sali(DP, prm, yg, wg, renorm_every=2, report=rep, **st).cpu().numpy()
+    assert (rep.status.cpu().numpy() == 0).all() and (rep.t_final.cpu().numpy() == 30.0).all()
+    assert rel_state(yg.cpu().numpy(), yo).max() <= 1e-8
+    reg = ro["series"][0] > 1e-4
+    assert reg.sum() > 0.5 * n_ic and np.abs(sg[0][reg] / ro["series"][0][reg] - 1).max() <= 1e-5
+    assert abs(rep.n_accepted.cpu().numpy().sum() / ro["n_accepted"].sum() - 1) <= 1e-2
+    for k in (1, 4):
+        wk = np.ascontiguousarray(w4[:k])
+        lo = orc.lyap(DP, prm, y0.copy(), wk.copy(), renorm_every=3, precision="f80", **st)["lam"]
+        lg = chs.lyap(DP, prm, dev(y0), dev(wk), renorm_every=3, **st).cpu().numpy()
+        assert lam_err(lg, lo, 30.0) <= 1e-5, k
+    # regular / chaotic classification over a long horizon on an ensemble that mixes both (energies from
+    # libration to tumbling): class agreement with the oracle >= 99.9 % (here: all but none of 400)
+    y1 = W.double_pendulum_ics(400, seed=9, theta_max=3.0, p_max=0.5)
+    w1 = W.deviation_vectors(400, 2, 4, 45, "unit")
+    so = orc.sali(DP, prm, y1.copy(), w1.copy(), renorm_every=1, h=0.01, n_steps=40000, precision="f64")["series"][0]
+    sg = chs.sali(DP, prm, dev(y1), dev(w1), renorm_every=1, h=0.01, n_steps=40000).cpu().numpy()[0]
+    cls_o, cls_g = so < 1e-8, sg < 1e-8
+    assert 0.1 < cls_o.mean() < 0.9
+    clear = (so < 1e-12) | (so > 1e-4)            # away from the threshold both sides must agree
+    assert (cls_o[clear] == cls_g[clear]).all() and (cls_o == cls_g).mean() >= 0.99
+    # the entry points that have no compiled kernel still say so
+    with pytest.raises(chs.ChaoticusError):
+        chs.gali(DP, prm, dev(y0), dev(w2), renorm_every=1, **st)
