@@ -47,7 +47,8 @@ typedef enum { CHS_OK = 0, CHS_EINVAL = 1, CHS_EUNSUPPORTED = 2, CHS_ECUDA = 3 }
  *  CHS_SYS_FPUT          n = 2N, params (N, k, alpha, beta), N given as a double, fixed ends
  *                        q_0 = q_{N+1} = 0, N+1 springs.  PAPER.md:98 Eq.(6),
  *                        PAPER.md:103-106 Eq.(7), Eq.(8).  Compiled: every N from 1 to 256
- *                        (integration, LD, SALI, GALI_4, Lyapunov k = 4; N = 8 also GALI_2,3 and k = 1,2).
+ *                        (integration, LD, SALI, GALI_4, Lyapunov k = 4; N = 8 also GALI_2,3 and k = 1,2);
+ *                        Lyapunov spectra on column blocks: k = 2N for N = 4, 8; k = 8 for N = 8, 16.
  *  CHS_SYS_DOUBLE_PENDULUM  n = 4, params (sigma, alpha) = (mass ratio, length ratio); state
  *                        (theta1, theta2, p1, p2).  NOT separable: Eq.(1)
  *                        Eq.(2), Eq.(3); generic first-order kernels.  Integration (fixed,

@@ -17,7 +17,7 @@ BUILD = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libchaoticus.so")
 PROBE_LIB = os.path.join(HERE, "libchaoticus_probe.so")
 UNITS = ["chaoticus", "inst_hh", "inst_hh_ind", "inst_hh_adapt", "inst_hh_adapt2", "inst_c3", "inst_c3_lyap",
-         "inst_c3_more", "inst_dp", "inst_fput", "inst_fput_adapt",
+         "inst_c3_more", "inst_dp", "inst_fput", "inst_fput_adapt", "inst_fput_spec",
          "inst_fput_n4", "inst_fput_n8", "inst_fput_n16", "inst_fput_n32", "inst_fput_n64",
          "inst_fput_pad4", "inst_fput_pad8", "inst_fput_pad16", "inst_fput_pad32", "inst_fput_pad64",
          "inst_fput_wide64", "inst_fput_wide128", "inst_fput_wide256"]

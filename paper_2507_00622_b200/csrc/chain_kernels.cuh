@@ -23,54 +23,67 @@
 
 namespace chs {
 
-template <int LT, int PPL_, int K_, bool PAD_ = false, bool COLD_ = false>
+template <int LT, int PPL_, int K_, bool PAD_ = false, bool COLD_ = false, int NB_ = 1>
 struct Chain {
-    static constexpr int K = K_, L = LT, PPL = PPL_;
+    // NB > 1 ("column blocks", for spectra with more vectors than one lane's registers hold): the trajectory
+    // is owned by NB adjacent sub-tiles of LT lanes; each sub-tile integrates its own replica of the orbit
+    // (bit-identical: same operations on the same numbers) and K of the NB K deviation vectors; only the
+    // Gram-Schmidt step couples the sub-tiles, through shuffles over the whole group.
+    static constexpr int K = K_, PPL = PPL_, NB = NB_;
+    static constexpr int L = LT * NB;  // lanes per trajectory
+    static constexpr int KTOT = K * NB;
     static constexpr bool PAD = PAD_;
     static constexpr bool COLD = COLD_;  // carry words and log accumulators in shared memory
     static constexpr int NCOL = 1 + K;
     static constexpr int NI = NCOL * PPL;  // item v * PPL + j: column v (0 = orbit), local particle j
     static constexpr int NSLOT = LT * PPL;
     static constexpr int NCOMP = PPL;      // items 0..PPL-1: the orbit coordinates -- compensated update
+    static_assert(NB == 1 || L <= 32, "column blocks live in one warp");
     using Params = FputParams;
 
     Params prm;
-    int lt;
+    int lt;   // lane in the trajectory's group (0 .. L-1)
+    int lp;   // lane in the sub-tile = which particles (0 .. LT-1)
+    int blk;  // column block (0 .. NB-1)
     int np;   // real chain length (== NSLOT unless PAD)
     mutable int par;  // wide tiles: which half of the edge buffer the next exchange uses
     double q[NI], p[NI];
-    LogBank<NCOL, COLD> lg;  // deferred-log accumulators, v >= 1: identical on all lanes of the tile
+    LogBank<NCOL, COLD> lg;  // deferred-log accumulators, v >= 1: identical on all lanes of the sub-tile
 
     __device__ __forceinline__ void init(const Params& P) {
         prm = P;
         lt = (int)(threadIdx.x % L);
+        lp = lt % LT;
+        blk = lt / LT;
         np = PAD ? P.np : NSLOT;
         par = 0;
         lg.init();
     }
-    __device__ __forceinline__ double dcount() const { return (double)(2 * np * NCOL); }
-    __device__ __forceinline__ bool real(int j) const { return !PAD || lt * PPL + j < np; }
+    // global index (0-based) of this block's deviation column v >= 1
+    __device__ __forceinline__ int gcol(int v) const { return blk * K + (v - 1); }
+    __device__ __forceinline__ double dcount() const { return (double)(2 * np * (1 + KTOT)); }
+    __device__ __forceinline__ bool real(int j) const { return !PAD || lp * PPL + j < np; }
     __device__ __forceinline__ void reset_logs() { lg.init(); }
     __device__ __forceinline__ void load(const double* y, const double* w, long long n_ic, long long ic,
                                          double psign) {
         const int n = 2 * np;
 #pragma unroll
         for (int j = 0; j < PPL; j++) {
-            const int pi = lt * PPL + j;
+            const int pi = lp * PPL + j;
             const bool on = real(j);
             q[j] = on ? y[(long long)pi * n_ic + ic] : 0.0;
             p[j] = on ? psign * y[(long long)(np + pi) * n_ic + ic] : 0.0;
 #pragma unroll
             for (int v = 1; v < NCOL; v++) {
-                q[v * PPL + j] = on ? w[((long long)(v - 1) * n + pi) * n_ic + ic] : 0.0;
-                p[v * PPL + j] = on ? w[((long long)(v - 1) * n + np + pi) * n_ic + ic] : 0.0;
+                q[v * PPL + j] = on ? w[((long long)gcol(v) * n + pi) * n_ic + ic] : 0.0;
+                p[v * PPL + j] = on ? w[((long long)gcol(v) * n + np + pi) * n_ic + ic] : 0.0;
             }
         }
     }
     __device__ __forceinline__ void displace(int comp, double delta, double psign) {
 #pragma unroll
         for (int j = 0; j < PPL; j++) {
-            const int pi = lt * PPL + j;
+            const int pi = lp * PPL + j;
             if (!real(j)) continue;  // (a padded slot's index collides with a momentum component)
             if (comp == pi) q[j] += delta;
             if (comp == np + pi) p[j] += psign * delta;
@@ -80,22 +93,24 @@ struct Chain {
         const int n = 2 * np;
 #pragma unroll
         for (int j = 0; j < PPL; j++) {
-            const int pi = lt * PPL + j;
+            const int pi = lp * PPL + j;
             if (!real(j)) continue;
-            y[(long long)pi * n_ic + ic] = bad ? nan("") : q[j];
-            y[(long long)(np + pi) * n_ic + ic] = bad ? nan("") : p[j];
+            if (blk == 0) {  // every block holds the same orbit
+                y[(long long)pi * n_ic + ic] = bad ? nan("") : q[j];
+                y[(long long)(np + pi) * n_ic + ic] = bad ? nan("") : p[j];
+            }
 #pragma unroll
             for (int v = 1; v < NCOL; v++) {
-                w[((long long)(v - 1) * n + pi) * n_ic + ic] = bad ? nan("") : q[v * PPL + j];
-                w[((long long)(v - 1) * n + np + pi) * n_ic + ic] = bad ? nan("") : p[v * PPL + j];
+                w[((long long)gcol(v) * n + pi) * n_ic + ic] = bad ? nan("") : q[v * PPL + j];
+                w[((long long)gcol(v) * n + np + pi) * n_ic + ic] = bad ? nan("") : p[v * PPL + j];
             }
         }
     }
     __device__ __forceinline__ void store_logs(const RunArgs& a, long long ic, bool bad, double elapsed) const {
-        if (lt != 0) return;
+        if (lp != 0) return;
 #pragma unroll
         for (int v = 1; v < NCOL; v++) {
-            const long long o = (long long)(v - 1) * a.n_ic + ic;
+            const long long o = (long long)gcol(v) * a.n_ic + ic;
             const double lv = lg.value(v);
             if (a.logacc) a.logacc[o] = bad ? nan("") : a.logacc[o] + lv;
             if (a.lambda) a.lambda[o] = (bad || elapsed == 0.0) ? nan("") : lv / fabs(elapsed);
@@ -106,7 +121,7 @@ struct Chain {
                                                double (&pc)[PPL]) const {
 #pragma unroll
         for (int j = 0; j < PPL; j++) {
-            const int pi = lt * PPL + j;
+            const int pi = lp * PPL + j;
             qc[j] = real(j) ? cw[(long long)pi * n_ic + ic] : 0.0;
             pc[j] = real(j) ? cw[(long long)(np + pi) * n_ic + ic] : 0.0;
         }
@@ -115,8 +130,8 @@ struct Chain {
                                                 const double (&pc)[PPL], bool bad) const {
 #pragma unroll
         for (int j = 0; j < PPL; j++) {
-            const int pi = lt * PPL + j;
-            if (!real(j)) continue;
+            const int pi = lp * PPL + j;
+            if (!real(j) || blk != 0) continue;
             cw[(long long)pi * n_ic + ic] = bad ? 0.0 : qc[j];
             cw[(long long)(np + pi) * n_ic + ic] = bad ? 0.0 : pc[j];
         }
@@ -134,19 +149,19 @@ struct Chain {
     // tile is the thread block): shuffles inside each warp, and the two edge lanes of every warp swap their
     // values through shared memory; the buffer alternates between calls, so one __syncthreads per call.
     __device__ __forceinline__ void exchange(const double (&Q)[NI], double (&xl)[NCOL], double (&xr)[NCOL]) const {
-        if constexpr (L <= 32) {
-            const bool first = (lt == 0), last = (lt == L - 1);
+        if constexpr (LT <= 32) {
+            const bool first = (lp == 0), last = (lp == LT - 1);
 #pragma unroll
             for (int v = 0; v < NCOL; v++) {
-                xl[v] = __shfl_up_sync(0xffffffffu, Q[v * PPL + PPL - 1], 1, L);
-                xr[v] = __shfl_down_sync(0xffffffffu, Q[v * PPL], 1, L);
+                xl[v] = __shfl_up_sync(0xffffffffu, Q[v * PPL + PPL - 1], 1, LT);
+                xr[v] = __shfl_down_sync(0xffffffffu, Q[v * PPL], 1, LT);
                 if (first) xl[v] = 0.0;
                 if (last) xr[v] = 0.0;
             }
         } else {
-            constexpr int W = L / 32;
+            constexpr int W = LT / 32;
             __shared__ double edge[2][NCOL][2][W];  // [parity][column][first / last particle of the warp][warp]
-            const int wid = lt >> 5, ln = lt & 31;
+            const int wid = lp >> 5, ln = lp & 31;
 #pragma unroll
             for (int v = 0; v < NCOL; v++) {
                 xl[v] = __shfl_up_sync(0xffffffffu, Q[v * PPL + PPL - 1], 1, 32);
@@ -212,7 +227,7 @@ struct Chain {
         double s = 0.0;
 #pragma unroll
         for (int j = 0; j < PPL; j++) s = fma(q[u * PPL + j], q[v * PPL + j], fma(p[u * PPL + j], p[v * PPL + j], s));
-        return tile_sum<L>(s);
+        return tile_sum<LT>(s);
     }
     __device__ __forceinline__ void scale(int v, double f) {
 #pragma unroll
@@ -233,21 +248,66 @@ struct Chain {
     }
     // modified Gram-Schmidt, right-looking order (see col_kernels.cuh)
     __device__ __forceinline__ void mgs(bool want_log, bool apply) {
+        if constexpr (NB == 1) {
 #pragma unroll
-        for (int v = 1; v < NCOL; v++) {
-            const double s = dot(v, v), ri = fast_rsqrt(s);
-            scale(v, apply ? ri : 1.0);
-            if (want_log && apply) lg.mul(v, s * ri);
+            for (int v = 1; v < NCOL; v++) {
+                const double s = dot(v, v), ri = fast_rsqrt(s);
+                scale(v, apply ? ri : 1.0);
+                if (want_log && apply) lg.mul(v, s * ri);
 #pragma unroll
-            for (int u = v + 1; u < NCOL; u++) {
-                double dt = dot(v, u);
-                if (!apply) dt = 0.0;
+                for (int u = v + 1; u < NCOL; u++) {
+                    double dt = dot(v, u);
+                    if (!apply) dt = 0.0;
 #pragma unroll
-                for (int j = 0; j < PPL; j++) {
-                    q[u * PPL + j] = fma(-dt, q[v * PPL + j], q[u * PPL + j]);
-                    p[u * PPL + j] = fma(-dt, p[v * PPL + j], p[u * PPL + j]);
+                    for (int j = 0; j < PPL; j++) {
+                        q[u * PPL + j] = fma(-dt, q[v * PPL + j], q[u * PPL + j]);
+                        p[u * PPL + j] = fma(-dt, p[v * PPL + j], p[u * PPL + j]);
+                    }
                 }
             }
+        } else {
+            // column blocks: global column g lives in block g / K as local column 1 + g % K.  It is broadcast
+            // to every block (lane (b, lp) reads lane (owner, lp)), normalised there redundantly (same numbers,
+            // same order: bit-identical), written back by its owner, and projected out of every later column.
+            static_for<0, KTOT>([&](auto gc) {
+                constexpr int g = decltype(gc)::value, owner = g / K, v = 1 + g % K;
+                double wq[PPL], wp[PPL];
+                double s = 0.0;
+#pragma unroll
+                for (int j = 0; j < PPL; j++) {
+                    wq[j] = __shfl_sync(0xffffffffu, q[v * PPL + j], owner * LT + lp, L);
+                    wp[j] = __shfl_sync(0xffffffffu, p[v * PPL + j], owner * LT + lp, L);
+                    s = fma(wq[j], wq[j], fma(wp[j], wp[j], s));
+                }
+                s = tile_sum<LT>(s);
+                const double ri = fast_rsqrt(s);
+#pragma unroll
+                for (int j = 0; j < PPL; j++) {
+                    wq[j] *= ri;
+                    wp[j] *= ri;
+                }
+                if (apply && blk == owner) {
+#pragma unroll
+                    for (int j = 0; j < PPL; j++) {
+                        q[v * PPL + j] = wq[j];
+                        p[v * PPL + j] = wp[j];
+                    }
+                    if (want_log) lg.mul(v, s * ri);
+                }
+#pragma unroll
+                for (int u = 1; u < NCOL; u++) {
+                    double d = 0.0;
+#pragma unroll
+                    for (int j = 0; j < PPL; j++) d = fma(wq[j], q[u * PPL + j], fma(wp[j], p[u * PPL + j], d));
+                    d = tile_sum<LT>(d);
+                    if (!(apply && gcol(u) > g)) d = 0.0;
+#pragma unroll
+                    for (int j = 0; j < PPL; j++) {
+                        q[u * PPL + j] = fma(-d, wq[j], q[u * PPL + j]);
+                        p[u * PPL + j] = fma(-d, wp[j], p[u * PPL + j]);
+                    }
+                }
+            });
         }
     }
     template <int MODE>
@@ -262,6 +322,7 @@ struct Chain {
     // loop is made warp-uniform with a vote).
     template <int IND>
     __device__ __forceinline__ double indicator() const {
+        static_assert(IND == IND_NONE || NB == 1, "SALI / GALI are evaluated inside one sub-tile");
         if constexpr (IND == IND_SALI) {
             constexpr int b = (K >= 2 ? 2 : 1);
             double sp = 0.0, sm = 0.0;

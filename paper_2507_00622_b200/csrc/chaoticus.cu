@@ -155,7 +155,8 @@ int first_of(const chs::LaunchReq& rq, std::initializer_list<Launcher> ls) {
 int dispatch_fput(const chs::LaunchReq& rq) {
     using namespace chs;
     const int N = rq.fput_n;
-    int r = -1;
+    int r = try_launch_fput_spec(rq);  // spectra on column blocks
+    if (r != -1) return r;
     switch (N) {  // exact tiles
         case 4: r = try_launch_fput_n4(rq); break;
         case 8: r = first_of(rq, {try_launch_fput_n8, try_launch_fput8_more, try_launch_fput8_adapt}); break;

@@ -46,6 +46,23 @@ int run_chain_ld_t(const LaunchReq& rq) {
     return (int)cudaGetLastError();
 }
 
+// Lyapunov spectrum with NB K vectors on NB column blocks (chain_kernels.cuh): fixed step, Gram-Schmidt
+template <int LT, int PPL, bool PAD, int KB, int NB, int TPB, int MINB, bool COLD = false>
+int run_chain_blocks(const LaunchReq& rq) {
+    FputParams prm;
+    if (!fput_params(rq, prm)) return (int)cudaErrorInvalidValue;
+    if (rq.fput_n > LT * PPL || (!PAD && rq.fput_n != LT * PPL)) return (int)cudaErrorInvalidValue;
+    using C = Chain<LT, PPL, KB, PAD, COLD, NB>;
+    auto kern = run_kernel<C, MODE_MGS, IND_NONE, false, TPB, MINB>;
+    const long long n_threads = rq.args.n_ic * C::L;
+    int r = finish_launch(rq, kern, TPB, C::L, n_threads);
+    if (r != -2) return r;
+    const long long blocks = (n_threads + TPB - 1) / TPB;
+    if (blocks == 0) return 0;
+    kern<<<(unsigned)blocks, TPB, 0, rq.stream>>>(rq.tab, prm, rq.args);
+    return (int)cudaGetLastError();
+}
+
 // the kernel set every tile class has: integration (fixed, adaptive), LD, SALI, GALI_4 (fixed, adaptive),
 // Lyapunov k = 4.  Returns -1 for anything else.
 template <int NS, bool PAD>

@@ -38,6 +38,7 @@ int try_launch_dp(const LaunchReq& rq);
 // FPUT: by chain length (fput_launch.h "tile classes")
 int try_launch_fput8_more(const LaunchReq& rq);
 int try_launch_fput8_adapt(const LaunchReq& rq);
+int try_launch_fput_spec(const LaunchReq& rq);
 int try_launch_fput_n4(const LaunchReq& rq);
 int try_launch_fput_n8(const LaunchReq& rq);
 int try_launch_fput_n16(const LaunchReq& rq);

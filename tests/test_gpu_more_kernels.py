@@ -530,3 +530,43 @@ def test_double_pendulum_adaptive_and_classification(chs, orc):
     # the entry points that have no compiled kernel still say so
     with pytest.raises(chs.ChaoticusError):
         chs.gali(DP, prm, dev(y0), dev(w2), renorm_every=1, **st)
+
+
+# ---------------------------------------------------------------------------- spectra on column blocks
+@pytest.mark.parametrize("N,k", [(4, 8), (8, 8), (8, 16), (16, 8)])
+def test_fput_spectrum_column_blocks(chs, orc, N, k):
+    """Lyapunov spectra with more vectors than one lane holds: column blocks of 4 vectors on
+    adjacent sub-tiles, each with its own bit-identical replica of the orbit; Gram-Schmidt across the
+    blocks by shuffles.  Full spectra (k = 2N): exponents sum to zero and pair up."""
+    n_ic = 37                                            # ragged
+    prm = W.fput_params(N, 1.0, 0.1, 0.8)
+    y0 = W.fput_ics(n_ic, N, seed=20 + N, E=0.3 * N)
+    w0 = W.deviation_vectors(n_ic, k, 2 * N, 70 + N, "raw")      # not orthonormal: the entry MGS is exercised
+    info = chs.kernel_info(FPUT, prm, chs.WHAT_LYAP, k=k, n_ic=n_ic)
+    assert info["lanes"] == N * k // 4 and info["spill_bytes"] == 0
+    yo, wo, so = y0.copy(), w0.copy(), np.zeros((k, n_ic))
+    ro = orc.lyap(FPUT, prm, yo, wo, renorm_every=10, logsum=so, h=0.05, n_steps=1203, precision="f80")["lam"]
+    yg, wg, sg = dev(y0), dev(w0), dev(np.zeros((k, n_ic)))
+    lam = chs.lyap(FPUT, prm, yg, wg, renorm_every=10, logsum=sg, h=0.05, n_steps=1203).cpu().numpy()
+    assert lam_err(lam, ro, 0.05 * 1203) <= 1e-8
+    assert np.abs(sg.cpu().numpy() - so).max() <= 1e-9
+    assert rel_state(yg.cpu().numpy(), yo).max() <= 1e-10
+    assert np.abs(wg.cpu().numpy() - wo).max() <= 1e-9
+    Wm = np.transpose(wg.cpu().numpy(), (2, 0, 1))       # orthonormal on return
+    assert np.abs(Wm @ np.transpose(Wm, (0, 2, 1)) - np.eye(k)).max() <= 1e-13
+    if k == 2 * N:
+        assert np.abs(lam.sum(0)).max() <= 1e-11         # Liouville
+    # the first 4 exponents are those of the k = 4 kernel (same Gram-Schmidt prefix)
+    w4 = np.ascontiguousarray(w0[:4])
+    lam4 = chs.lyap(FPUT, prm, dev(y0), dev(w4), renorm_every=10, h=0.05, n_steps=1203).cpu().numpy()
+    assert np.abs(lam4 - lam[:4]).max() <= 1e-10
+    # bit-identical continuation
+    import torch
+    b_y, b_w = dev(y0), dev(w0)
+    rep = chs.Report(n_ic, "cuda", n=2 * N)
+    chs.lyap(FPUT, prm, b_y, b_w, renorm_every=10, h=0.05, n_steps=500, report=rep)
+    rep.resume = True
+    chs.lyap(FPUT, prm, b_y, b_w, renorm_every=10, t0=25.0, h=0.05, n_steps=703, report=rep)
+    a_y, a_w = dev(y0), dev(w0)
+    chs.lyap(FPUT, prm, a_y, a_w, renorm_every=10, h=0.05, n_steps=1203)
+    assert torch.equal(a_y, b_y)
