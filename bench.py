@@ -76,6 +76,7 @@ def parse(argv=None):
     ap.add_argument("--n-ic", type=int, default=1000, help="F3: ensemble size (PAPER.md:129: 10^3 random ICs)")
     ap.add_argument("--ldn-sigma", type=float, default=1e-3, help="LDN: neighbour displacement")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-sweeps", action="store_true", help="skip the FPUT DoF and ensemble-size sweeps of the headline line")
     ap.add_argument("--tune", type=int, default=0, help="development: kernel variant knob (chaoticus_set_option)")
     return ap.parse_args(argv)
 
@@ -522,6 +523,48 @@ def measure_config(chs, torch, flush, args, name, dfma_tflops, orc):
     return ent
 
 
+def run_sweeps(chs, torch, flush, args):
+    """Shapes of the paper's figures, driver-timed (one warm-up + 2 timed runs each, median):
+    fput_dof      PAPER.md:113, 129 (Fig. 3): FPUT-beta, GALI_4, adaptive DOP8(5) rtol = atol = 1e-8 on a
+                  SATURATING ensemble (65536 ICs, t = 100) as a function of the chain length N -- the
+                  "linear trend" in the number of degrees of freedom; N spans every tile class (exact and
+                  padded in-warp tiles, wide tiles);
+    ensemble_size PAPER.md:94, 125 (Fig. 2): the fixed-step SALI kernel, time per IC against the number of
+                  simultaneously integrated ICs."""
+    out = {"fput_dof": [], "ensemble_size": []}
+    for N in (4, 8, 12, 16, 32, 48, 64, 128):
+        a2 = argparse.Namespace(**vars(args))
+        a2.workload, a2.fput_n, a2.n_ic, a2.shrink, a2.shrink_ic = "F3", N, 65536, 10, 1
+        wk = make_workload(chs, torch, a2, 0, 1, "F3")
+        wk["prepare"]()
+        wk["step_dev"]()
+        ms = timed(torch, flush, wk, 2)
+        rk = resolve_rk_steps(wk["wl"])
+        med = float(np.median(ms))
+        out["fput_dof"].append({"N": N, "n_ic": 65536, "t_end": 100.0, "ms": med, "ms_per_dof": med / N,
+                                "accepted": wk["wl"]["accepted"], "rejected": wk["wl"]["rejected"],
+                                "attempts_per_s": rk / (med * 1e-3), "lanes": wk["kinfo"]["lanes"],
+                                "regs": wk["kinfo"]["regs"], "spill_bytes": wk["kinfo"]["spill_bytes"]})
+        del wk
+        torch.cuda.empty_cache()
+    for side, ns in ((32, 10000), (64, 10000), (128, 10000), (256, 10000), (512, 2000), (1024, 2000)):
+        a2 = argparse.Namespace(**vars(args))
+        a2.workload, a2.sali_side, a2.sali_steps = "C1sat", side, ns
+        wk = make_workload(chs, torch, a2, 0, 1, "C1sat")
+        wk["prepare"]()
+        wk["step_dev"]()
+        ms = timed(torch, flush, wk, 2)
+        med = float(np.median(ms))
+        rk = wk["wl"]["rk_steps"]
+        out["ensemble_size"].append({"n_ic": side * side, "n_steps": ns, "ms": med,
+                                     "ns_per_ic_per_step": 1e6 * med / rk, "rk_steps_per_s": rk / (med * 1e-3),
+                                     "frac_of_fp64_peak": FLOP_PER_STEP["C1sat"] * rk / (med * 1e-3) / 1e12 / NOMINAL_FP64_TFLOPS,
+                                     "lanes": wk["kinfo"]["lanes"]})
+        del wk
+        torch.cuda.empty_cache()
+    return out
+
+
 def main(argv=None):
     argv = sys.argv[1:] if argv is None else argv
     args = parse(argv)
@@ -658,6 +701,8 @@ def main(argv=None):
                         per[name]["cpu_baseline"] = out["cpu_baseline"]
                     continue
                 per[name] = measure_config(chs, torch, flush, args, name, dfma_tflops, orc)
+            if not args.no_sweeps:
+                out["sweeps"] = run_sweeps(chs, torch, flush, args)
         out["per_config"] = per
         out["per_config_clocks"] = cs2.summary()
         out["gpu_launches_total"] = out["gpu_launches"] + sum(2 + args.config_steps + 4 for n in names if n != "C2")

@@ -58,6 +58,7 @@ struct Chain {
         np = PAD ? P.np : NSLOT;
         par = 0;
         lg.init();
+        init_walls();
     }
     // global index (0-based) of this block's deviation column v >= 1
     __device__ __forceinline__ int gcol(int v) const { return blk * K + (v - 1); }
@@ -145,9 +146,8 @@ struct Chain {
     }
 
     // xl[v] = the left neighbour's last particle of column v (0 at the left wall), xr[v] = the right
-    // neighbour's first particle (0 at the right wall).  In-warp tiles: shuffles.  Wide tiles (L > 32, the
-    // tile is the thread block): shuffles inside each warp, and the two edge lanes of every warp swap their
-    // values through shared memory; the buffer alternates between calls, so one __syncthreads per call.
+    // neighbour's first particle (0 at the right wall).  In-warp tiles: shuffles.  Wide tiles (LT > 32, the
+    // tile is the thread block): through shared memory.
     __device__ __forceinline__ void exchange(const double (&Q)[NI], double (&xl)[NCOL], double (&xr)[NCOL]) const {
         if constexpr (LT <= 32) {
             const bool first = (lp == 0), last = (lp == LT - 1);
@@ -159,23 +159,46 @@ struct Chain {
                 if (last) xr[v] = 0.0;
             }
         } else {
-            constexpr int W = LT / 32;
-            __shared__ double edge[2][NCOL][2][W];  // [parity][column][first / last particle of the warp][warp]
-            const int wid = lp >> 5, ln = lp & 31;
+            // wide tile: every thread posts its first and last particle of each column in shared memory
+            // ([half][column][slot], slot = lp + 1; slots 0 and LT + 1 are the walls and stay zero), one
+            // __syncthreads, then reads its two neighbours' -- no branch, no lane is special
+            double* bf = edge_first();
+            double* bl = (PPL == 1) ? bf : edge_last();
 #pragma unroll
             for (int v = 0; v < NCOL; v++) {
-                xl[v] = __shfl_up_sync(0xffffffffu, Q[v * PPL + PPL - 1], 1, 32);
-                xr[v] = __shfl_down_sync(0xffffffffu, Q[v * PPL], 1, 32);
-                if (ln == 0) edge[par][v][0][wid] = Q[v * PPL];
-                if (ln == 31) edge[par][v][1][wid] = Q[v * PPL + PPL - 1];
+                bf[(par * NCOL + v) * (LT + 2) + lp + 1] = Q[v * PPL];
+                if constexpr (PPL > 1) bl[(par * NCOL + v) * (LT + 2) + lp + 1] = Q[v * PPL + PPL - 1];
             }
             __syncthreads();
 #pragma unroll
             for (int v = 0; v < NCOL; v++) {
-                if (ln == 0) xl[v] = (wid > 0) ? edge[par][v][1][wid - 1] : 0.0;
-                if (ln == 31) xr[v] = (wid < W - 1) ? edge[par][v][0][wid + 1] : 0.0;
+                xl[v] = bl[(par * NCOL + v) * (LT + 2) + lp];
+                xr[v] = bf[(par * NCOL + v) * (LT + 2) + lp + 2];
             }
             par ^= 1;
+        }
+    }
+    // the wide tile's exchange buffers (two halves: the buffer alternates between calls, so one barrier
+    // per call is enough) and their wall slots
+    __device__ __forceinline__ static double* edge_first() {
+        __shared__ double b[2 * NCOL * (LT + 2)];
+        return b;
+    }
+    __device__ __forceinline__ static double* edge_last() {
+        __shared__ double b[(PPL > 1 ? 2 * NCOL * (LT + 2) : 1)];
+        return b;
+    }
+    __device__ __forceinline__ void init_walls() const {
+        if constexpr (LT > 32) {
+            if (lp < 2 * NCOL) {  // slots 0 and LT + 1 of every (half, column)
+                edge_first()[lp * (LT + 2)] = 0.0;
+                edge_first()[lp * (LT + 2) + LT + 1] = 0.0;
+                if constexpr (PPL > 1) {
+                    edge_last()[lp * (LT + 2)] = 0.0;
+                    edge_last()[lp * (LT + 2) + LT + 1] = 0.0;
+                }
+            }
+            __syncthreads();
         }
     }
 
@@ -239,11 +262,22 @@ struct Chain {
 
     // w_v <- w_v/|w_v|, lg_v += ln|w_v|
     __device__ __forceinline__ void renorm(bool want_log, bool apply) {
+        if constexpr (K > 0) {
+            double s2[K];
 #pragma unroll
-        for (int v = 1; v < NCOL; v++) {
-            const double s = dot(v, v), ri = fast_rsqrt(s);
-            scale(v, apply ? ri : 1.0);
-            if (want_log && apply) lg.mul(v, s * ri);
+            for (int v = 1; v < NCOL; v++) {
+                double s = 0.0;
+#pragma unroll
+                for (int j = 0; j < PPL; j++) s = fma(q[v * PPL + j], q[v * PPL + j], fma(p[v * PPL + j], p[v * PPL + j], s));
+                s2[v - 1] = s;
+            }
+            tile_sum_vec<LT, K>(s2);  // all K squared norms in one reduction
+#pragma unroll
+            for (int v = 1; v < NCOL; v++) {
+                const double s = s2[v - 1], ri = fast_rsqrt(s);
+                scale(v, apply ? ri : 1.0);
+                if (want_log && apply) lg.mul(v, s * ri);
+            }
         }
     }
     // modified Gram-Schmidt, right-looking order (see col_kernels.cuh)

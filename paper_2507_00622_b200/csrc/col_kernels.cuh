@@ -703,8 +703,12 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
             dop8_solution<NI, C::NCOMP, false>(tab, h, h * h, s.q, s.p, F, qn, pn, qc, pc, qcn, pcn);
             double S5, S3;
             dop8_error_sums<NI>(tab, h, s.q, s.p, qn, pn, F, a.rtol, a.atol, on, S5, S3);
-            S5 = tile_sum<L>(S5);
-            S3 = tile_sum<L>(S3);
+            {
+                double S[2] = {S5, S3};
+                tile_sum_vec<L, 2>(S);
+                S5 = S[0];
+                S3 = S[1];
+            }
             const double err = (S5 == 0.0 && S3 == 0.0) ? 0.0 : h_try * S5 * fast_rsqrt((S5 + 0.01 * S3) * s.dcount());
 
             bool ren = false;

@@ -82,7 +82,7 @@ __device__ __forceinline__ double tile_sum(double x) {  // butterfly: identical 
         __shared__ double part[L / 32];
 #pragma unroll
         for (int d = 16; d >= 1; d >>= 1) x += __shfl_xor_sync(0xffffffffu, x, d, 32);
-        if ((threadIdx.x & 31u) == 0u) part[threadIdx.x >> 5] = x;
+        part[threadIdx.x >> 5] = x;  // every lane of a warp holds the same sum: no lane is special, no branch
         __syncthreads();
         x = part[0];
 #pragma unroll
@@ -90,6 +90,32 @@ __device__ __forceinline__ double tile_sum(double x) {  // butterfly: identical 
         __syncthreads();
     }
     return x;
+}
+// NV sums at once (renormalisation: the K squared norms; adaptive step: S5 and S3): the wide tile pays its
+// two barriers once instead of NV times; in-warp tiles: NV independent butterflies
+template <int L, int NV>
+__device__ __forceinline__ void tile_sum_vec(double (&x)[NV]) {
+    if constexpr (L <= 32) {
+#pragma unroll
+        for (int v = 0; v < NV; v++) x[v] = tile_sum<L>(x[v]);
+    } else {
+        __shared__ double part[NV][L / 32];
+#pragma unroll
+        for (int v = 0; v < NV; v++) {
+#pragma unroll
+            for (int d = 16; d >= 1; d >>= 1) x[v] += __shfl_xor_sync(0xffffffffu, x[v], d, 32);
+            part[v][threadIdx.x >> 5] = x[v];
+        }
+        __syncthreads();
+#pragma unroll
+        for (int v = 0; v < NV; v++) {
+            double t = part[v][0];
+#pragma unroll
+            for (int w = 1; w < L / 32; w++) t += part[v][w];
+            x[v] = t;
+        }
+        __syncthreads();
+    }
 }
 template <int L>
 __device__ __forceinline__ bool tile_any(bool b) {
