@@ -77,7 +77,6 @@ def parse(argv=None):
     ap.add_argument("--ldn-sigma", type=float, default=1e-3, help="LDN: neighbour displacement")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sweeps", action="store_true", help="skip the FPUT DoF and ensemble-size sweeps of the headline line")
-    ap.add_argument("--tune", type=int, default=0, help="development: kernel variant knob (chaoticus_set_option)")
     return ap.parse_args(argv)
 
 
@@ -595,8 +594,6 @@ def main(argv=None):
             dist.barrier()
         torch.cuda.synchronize()
 
-    if args.tune:
-        chs.set_option("tune", args.tune)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
     wk = make_workload(chs, torch, args, rank, world)
     wl, step_dev, step_e2e, h2d, d2h, kinfo = wk["wl"], wk["step_dev"], wk["step_e2e"], wk["h2d"], wk["d2h"], wk["kinfo"]

@@ -21,7 +21,6 @@ thread_local char g_err[512] = "";
 // right after the kernel launch and is handed out again only once that event has completed.  When every
 // slot is busy the call runs without refill (one trajectory per tile: same results, bit for bit).
 std::atomic<int> g_adaptive_refill{1};
-std::atomic<int> g_tune{0};
 constexpr int kQueueSlots = 64, kMaxDevices = 64;
 struct QueuePool {
     unsigned long long* base = nullptr;  // kQueueSlots device counters (cudaMalloc, never freed)
@@ -248,7 +247,6 @@ int run_common(int what, const chs_problem* pb, long long n_ic, double* y, doubl
     rq.tab = make_tab(st->adaptive ? 1.0 : st->h);
     rq.stream = (cudaStream_t)stream;
     rq.info = info;
-    rq.tune = g_tune.load();
     chs::RunArgs& a = rq.args;
     a.n_ic = n_ic;
     a.y = y;
@@ -295,10 +293,6 @@ int chaoticus_version(void) { return CHAOTICUS_VERSION; }
 int chaoticus_set_option(const char* name, int value) {
     if (name && std::strcmp(name, "adaptive_refill") == 0) {
         g_adaptive_refill.store(value != 0 ? 1 : 0);
-        return CHS_OK;
-    }
-    if (name && std::strcmp(name, "tune") == 0) {
-        g_tune.store(value);
         return CHS_OK;
     }
     return fail(CHS_EINVAL, "unknown option '%s'", name ? name : "(null)");

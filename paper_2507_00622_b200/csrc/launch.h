@@ -23,7 +23,6 @@ struct LaunchReq {
     KernelInfo* info;  // non-null: report the launch shape, launch nothing
     // LD: which directions
     int dir_first, n_dirs;
-    int tune;  // development knob (chaoticus_set_option("tune", v)): selects a kernel variant where one exists
 };
 
 // each returns -1 if it has no kernel for the request, else a cudaError_t (0 = success)
