@@ -680,7 +680,7 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
 
             bool active = !done && status == ST_OK && dir * (a.t_end - t) > 0.0;
             if (!rejected) {
-                min_step = 10.0 * fabs(nextafter(t, dir * INFINITY) - t);
+                min_step = ten_ulp(t, dir);  // 10 |nextafter(t, dir inf) - t|
                 h_abs = fmax(h_abs, min_step);
             }
             if (active && h_abs < min_step) {
@@ -709,43 +709,48 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
                 S5 = S[0];
                 S3 = S[1];
             }
-            const double err = (S5 == 0.0 && S3 == 0.0) ? 0.0 : h_try * S5 * fast_rsqrt((S5 + 0.01 * S3) * s.dcount());
-
+            // err = |h| S5 / sqrt(D (S5 + 0.01 S3)) against 1, and the step-size factor 0.9 err^(-1/8), without
+            // forming err (dop8_core.cuh "step-size controller"): accept <=> num^2 < den.  The whole decision is
+            // written with selects, not branches: one basic block, so the short controller chain, the commit and
+            // (thread layout) the renormalisation of the new vectors are scheduled side by side.
+            const double num = h_try * S5, den = fma(0.01, S3, S5) * s.dcount(), num2 = num * num;
+            const bool zero = (S5 == 0.0) && (S3 == 0.0);          // err = 0
+            const bool acc = active && (zero || num2 < den);
+            const bool rej = active && !zero && num2 >= den;
+            if (active && !acc && !rej) status = ST_NONFINITE;       // NaN: inf or NaN in y+ (fast_rcp(inf) is NaN)
+            const float ff = step_factor(num2, den);
+            const double fd = (double)ff;
+            const float cap = rejected ? 1.0f : 10.0f;               // <= 1 right after a rejection
+            const double f_acc = (zero || !(ff < cap)) ? (double)cap : fd;
+            const double f_rej = (ff > 0.2f) ? fd : 0.2;
+            if (acc || rej) h_abs = h_try * (acc ? f_acc : f_rej);
+            rejected = rej ? true : (acc ? false : rejected);
+            n_acc += acc ? 1 : 0;
+            n_rej += rej ? 1 : 0;
+            t = acc ? t_new : t;
+#pragma unroll
+            for (int c = 0; c < NI; c++) {
+                s.q[c] = acc ? qn[c] : s.q[c];
+                s.p[c] = acc ? pn[c] : s.p[c];
+            }
+#pragma unroll
+            for (int c = 0; c < NC; c++) {
+                qc[c] = acc ? qcn[c] : qc[c];
+                pc[c] = acc ? pcn[c] : pc[c];
+            }
             bool ren = false;
-            if (active) {
-                if (err < 1.0) {
-                    double factor = (err == 0.0) ? 10.0 : fmin(10.0, 0.9 * inv_root8(err));
-                    if (rejected) factor = fmin(factor, 1.0);
-                    h_abs = h_try * factor;
-                    t = t_new;
-#pragma unroll
-                    for (int c = 0; c < NI; c++) {
-                        s.q[c] = qn[c];
-                        s.p[c] = pn[c];
-                    }
-#pragma unroll
-                    for (int c = 0; c < NC; c++) {
-                        qc[c] = qcn[c];
-                        pc[c] = pcn[c];
-                    }
-                    n_acc++;
-                    rejected = false;
+            if constexpr (MODE != MODE_NONE) {
+                if (acc) {
                     const bool at_end = !(dir * (a.t_end - t) > 0.0);
-                    if (MODE != MODE_NONE && (--cd == 0 || at_end)) {
+                    if (--cd == 0 || at_end) {
                         cd = a.m;
                         ren = true;
                     }
-                } else if (err >= 1.0) {
-                    h_abs = h_try * fmax(0.2, 0.9 * inv_root8(err));
-                    rejected = true;
-                    n_rej++;
-                } else {
-                    // inf or NaN in y+ makes its error scale, hence err, NaN (fast_rcp(inf) is NaN)
-                    status = ST_NONFINITE;
                 }
-            }
-            if constexpr (MODE != MODE_NONE) {
-                if (group_any<L>(ren)) {
+                // thread layout: renormalising is lane-local and cheap, so it runs every attempt under the
+                // predicate (no branch between it and the controller); tiles shuffle: only when some tile wants it
+                constexpr bool ALWAYS = (L == 1) && (MODE == MODE_NORM);
+                if (ALWAYS || group_any<L>(ren)) {
                     s.template do_renorm<MODE>(want_log, ren);
                     if (ren) s.scrub_carry(qc, pc);
                 }

@@ -375,8 +375,10 @@ __device__ __forceinline__ void dop8_error_sums(const Tab& tab, double h, const 
                                                 const double (&pn)[NI], const double (&F)[12][NI],
                                                 double rtol, double atol, const bool (&on)[NI], double& S5,
                                                 double& S3) {
-    S5 = 0.0;
-    S3 = 0.0;
+    // NACC interleaved partial sums (items c, c + NACC, ... go to sum c % NACC): the dependent chain is
+    // 2 NI / NACC fused multiply-adds deep instead of 2 NI (the error norm is on the serial tail of an attempt)
+    constexpr int NACC = NI < 3 ? NI : 3;
+    double a5[NACC], a3[NACC];
 #pragma unroll
     for (int c = 0; c < NI; c++) {
         double s5q = tab.e5q[0] * F[0][c], s3q = tab.e3q[0] * F[0][c];
@@ -391,19 +393,68 @@ __device__ __forceinline__ void dop8_error_sums(const Tab& tab, double h, const 
         double iq = fast_rcp(fma(rtol, fmax(fabs(q[c]), fabs(qn[c])), atol));
         double ip = fast_rcp(fma(rtol, fmax(fabs(p[c]), fabs(pn[c])), atol));
         double a = h * s5q * iq, b = s5p * ip, c3 = h * s3q * iq, d3 = s3p * ip;
-        if (on[c]) {
-            S5 = fma(a, a, fma(b, b, S5));
-            S3 = fma(c3, c3, fma(d3, d3, S3));
+        if (c < NACC) {
+            a5[c % NACC] = on[c] ? fma(a, a, b * b) : 0.0;
+            a3[c % NACC] = on[c] ? fma(c3, c3, d3 * d3) : 0.0;
+        } else if (on[c]) {
+            a5[c % NACC] = fma(a, a, fma(b, b, a5[c % NACC]));
+            a3[c % NACC] = fma(c3, c3, fma(d3, d3, a3[c % NACC]));
         }
+    }
+    S5 = a5[0];
+    S3 = a3[0];
+#pragma unroll
+    for (int k = 1; k < NACC; k++) {
+        S5 += a5[k];
+        S3 += a3[k];
     }
 }
 
 // per-trajectory status words (include/chaoticus.h CHS_ST_*)
 enum : int { ST_OK = 0, ST_NONFINITE = 1, ST_UNDERFLOW = 2, ST_MAXSTEPS = 3 };
 
-// x^(1/8) by three square roots (the controller's exponent)
+// x^(1/8) by three square roots (the starting step's exponent)
 __device__ __forceinline__ double root8(double x) { return sqrt(sqrt(sqrt(x))); }
-// x^(-1/8), x > 0 finite: branch-free (used once per attempt by the step-size controller)
+// x^(-1/8), x > 0 finite: branch-free (the generic first-order kernels' controller, gen_kernels.cuh)
 __device__ __forceinline__ double inv_root8(double x) { return fast_rsqrt(fast_sqrt(fast_sqrt(x))); }
+
+// ---- the step-size controller off the FP64 critical path ("Serial tail") ----
+// With num = |h| S5 and den = D (S5 + 0.01 S3) the error norm is err = num / sqrt(den), so
+//   accept  <=>  err < 1  <=>  num^2 < den            (no square root, no division), and
+//   0.9 err^(-1/8) = 0.9 (den / num^2)^(1/16)         (the factor the NEXT step size is multiplied by).
+// The factor only steers the step size (the accept test above is exact), so it is evaluated to single
+// precision: log2 of a double = its exponent (integer instructions) + MUFU.LG2 of its mantissa, one MUFU.EX2;
+// relative error ~3e-7.  This replaces 25 dependent FP64 instructions (one rsqrt for err, three for the
+// eighth root) by ~10 short-latency ones that do not touch the FP64 pipe.  Zero / subnormal / huge arguments
+// saturate into the clipping range [0.2, 10] on the correct side.
+__device__ __forceinline__ float log2_coarse(double x) {  // x >= 0
+    const int hi = __double2hiint(x);
+    const unsigned lo = (unsigned)__double2loint(x);
+    const float m = __int_as_float(0x3f800000 | ((hi & 0xfffff) << 3) | (int)(lo >> 29));  // mantissa in [1, 2)
+    float l;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l) : "f"(m));
+    return (float)(((hi >> 20) & 0x7ff) - 1023) + l;
+}
+__device__ __forceinline__ float step_factor(double num2, double den) {  // 0.9 (den/num2)^(1/16)
+    const float e = fmaf(log2_coarse(den) - log2_coarse(num2), 0.0625f, -0.15200309344504997f);  // + log2(0.9)
+    float f;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(f) : "f"(e));
+    return f;
+}
+
+// 10 |nextafter(t, dir inf) - t|: the smallest step the controller allows at time t (DESIGN.md "Adaptive
+// step", item 5).  The spacing of the doubles at t is 2^(e - 1075) (e: biased exponent), half of that when
+// t is a power of two and the step points towards zero; 10 x 2^k = 1.25 x 2^(k+3) is assembled from integer
+// instructions -- exact, and nothing on the FP64 pipe.  t = 0, subnormal or tiny t (result would be
+// subnormal), inf and NaN take the library route.
+__device__ __forceinline__ double ten_ulp(double t, double dir) {
+    const int hi = __double2hiint(t), lo = __double2loint(t);
+    const int e = (hi >> 20) & 0x7ff;
+    const bool pow2 = ((hi & 0xfffff) | lo) == 0;
+    const bool to_zero = (hi < 0) == (dir > 0.0);  // sign(t) opposite to the direction of integration
+    const int ef = e - 1075 + 3 + 1023 - ((pow2 && to_zero) ? 1 : 0);
+    if (e < 64 || e == 0x7ff) return 10.0 * fabs(nextafter(t, dir * INFINITY) - t);
+    return __hiloint2double((ef << 20) | 0x40000, 0);
+}
 
 }  // namespace chs
