@@ -205,7 +205,15 @@ struct Chain {
     // Eq.(7) with Eq.(8): p_i' = phi(Dq_{i+1}) - phi(Dq_i), Dq_i = q_i - q_{i-1}; variational:
     // dp_i' = g(Dq_{i+1}) dDq_{i+1} - g(Dq_i) dDq_i.  Springs s = 0..PPL of this lane: s = 0 to the left
     // neighbour (or the left wall), s = PPL to the right neighbour (or the right wall).
-    __device__ __forceinline__ void force(const double (&Q)[NI], double (&F)[NI]) const {
+    // sc: the factor the forces come out multiplied by (1, or h^2 in the adaptive kernels): it scales the
+    // spring constants once per attempt (the same products for all 12 stages), nothing per spring.
+    __device__ __forceinline__ void force(const double (&Q)[NI], double (&F)[NI], double sc = 1.0) const {
+        FputParams prm = this->prm;
+        prm.k *= sc;
+        prm.al *= sc;
+        prm.be *= sc;
+        prm.al2 *= sc;
+        prm.be3 *= sc;
         // all neighbour values first: 2 shuffles per column, none depends on arithmetic
         double xl[NCOL], xr[NCOL];
         exchange(Q, xl, xr);
@@ -241,9 +249,9 @@ struct Chain {
     }
 
     __device__ __forceinline__ void force2(const double (&Qa)[NI], double (&Fa)[NI], const double (&Qb)[NI],
-                                           double (&Fb)[NI]) const {
-        force(Qa, Fa);
-        force(Qb, Fb);
+                                           double (&Fb)[NI], double sc = 1.0) const {
+        force(Qa, Fa, sc);
+        force(Qb, Fb, sc);
     }
 
     __device__ __forceinline__ double dot(int u, int v) const {

@@ -245,13 +245,19 @@ struct Col {
     // column per lane the products of the lane's own x are formed while the orbit's coordinates Qo are
     // still in flight (Sys::pre / apply_pre): two or three dependent FMAs after the shuffle instead of four
     // levels (configs[0], 1024 ICs: 5.3 ms against 5.9 ms).
-    __device__ __forceinline__ void force(const double (&Q)[NI], double (&F)[NI]) const {
+    // g: the factor the forces come out multiplied by (1, or h^2 in the adaptive kernels: dop8_core.cuh
+    // dop8_stage_coords); where a Hessian is formed it absorbs g, so scaling costs nothing there.
+    __device__ __forceinline__ void force(const double (&Q)[NI], double (&F)[NI], double g = 1.0) const {
         if constexpr (L == 1) {
-            Sys::force(prm, &Q[0], &F[0]);
             if constexpr (CPL > 1) {
-                const typename Sys::Hess H = Sys::hess(prm, &Q[0], 1.0);
+                const typename Sys::Hess H = Sys::hess(prm, &Q[0], 1.0, g);
+                Sys::force_hess(prm, H, &Q[0], g, &F[0]);
 #pragma unroll
                 for (int j = 1; j < CPL; j++) Sys::apply(H, &Q[j * ND], &F[j * ND]);
+            } else {
+                Sys::force(prm, &Q[0], &F[0]);
+#pragma unroll
+                for (int d = 0; d < ND; d++) F[d] *= g;
             }
         } else if constexpr (CPL == 1) {
             const typename Sys::Pre P = Sys::pre(prm, &Q[0], s_lane);
@@ -259,17 +265,19 @@ struct Col {
 #pragma unroll
             for (int d = 0; d < ND; d++) Qo[d] = tile_bcast<L>(Q[d], 0);
             Sys::apply_pre(prm, P, Qo, &F[0]);
+#pragma unroll
+            for (int d = 0; d < ND; d++) F[d] *= g;
         } else {  // several columns per lane: a Hessian serves them (fewer instructions; measured faster)
             double Qo[ND];
 #pragma unroll
             for (int d = 0; d < ND; d++) Qo[d] = tile_bcast<L>(Q[d], 0);
-            const typename Sys::Hess H0 = Sys::hess(prm, Qo, s_lane);
+            const typename Sys::Hess H0 = Sys::hess(prm, Qo, s_lane, g);
             Sys::apply(H0, &Q[0], &F[0]);
             if constexpr (ALONE) {  // lane 0's other slots are idle: the same Hessian for every slot of a lane
 #pragma unroll
                 for (int j = 1; j < CPL; j++) Sys::apply(H0, &Q[j * ND], &F[j * ND]);
             } else {
-                const typename Sys::Hess H1 = Sys::hess(prm, Qo, 1.0);
+                const typename Sys::Hess H1 = Sys::hess(prm, Qo, 1.0, g);
 #pragma unroll
                 for (int j = 1; j < CPL; j++) Sys::apply(H1, &Q[j * ND], &F[j * ND]);
             }
@@ -277,9 +285,9 @@ struct Col {
     }
     // two independent force evaluations (dop8_stages PAIR)
     __device__ __forceinline__ void force2(const double (&Qa)[NI], double (&Fa)[NI], const double (&Qb)[NI],
-                                           double (&Fb)[NI]) const {
-        force(Qa, Fa);
-        force(Qb, Fb);
+                                           double (&Fb)[NI], double g = 1.0) const {
+        force(Qa, Fa, g);
+        force(Qb, Fb, g);
     }
 
     // value of component cc (0..N-1) of column `col` (compile-time), on every lane of the tile
@@ -471,13 +479,19 @@ __device__ __forceinline__ double initial_step(const S& s, double interval, doub
 
 // functors handed to dop8_stages (plain structs: generic lambdas with array-reference
 // parameters of dependent extent crash cudafe++ 12.9)
-template <class C>
+// SCALED: the forces come out multiplied by g (= h^2 of the attempt; adaptive kernels)
+template <class C, bool SCALED = false>
 struct ForceFn {
     const C& s;
-    __device__ __forceinline__ void operator()(const double (&Q)[C::NI], double (&F)[C::NI]) const { s.force(Q, F); }
+    double g;
+    __device__ __forceinline__ void operator()(const double (&Q)[C::NI], double (&F)[C::NI]) const {
+        if constexpr (SCALED) s.force(Q, F, g);
+        else s.force(Q, F);
+    }
     __device__ __forceinline__ void pair(const double (&Qa)[C::NI], double (&Fa)[C::NI], const double (&Qb)[C::NI],
                                          double (&Fb)[C::NI]) const {
-        s.force2(Qa, Fa, Qb, Fb);
+        if constexpr (SCALED) s.force2(Qa, Fa, Qb, Fb, g);
+        else s.force2(Qa, Fa, Qb, Fb);
     }
 };
 struct NoHook {
@@ -522,7 +536,7 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
 
     C s;
     s.init(prm);
-    const ForceFn<C> force{s};
+    const ForceFn<C> force{s, 1.0};
     const NoHook nohook{};
 
     long long n_acc = 0, n_rej = 0;
@@ -559,7 +573,7 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
         }
         for (long long st = 1; st <= a.n_steps; ++st) {
             double F[12][NI];
-            dop8_stages<NI, true, PAIR>(tab, 0.0, 0.0, s.q, s.p, F, force, nohook);
+            dop8_stages<NI, PAIR>(tab, s.q, s.p, F, force, nohook);
             double qn[NI], pn[NI];
             if constexpr (COLD) {
 #pragma unroll
@@ -568,7 +582,7 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
                     pc[c] = cold_carry[(NC + c) * kMaxTpb + threadIdx.x];
                 }
             }
-            dop8_solution<NI, C::NCOMP, true>(tab, 0.0, 0.0, s.q, s.p, F, qn, pn, qc, pc, qcn, pcn);
+            dop8_solution<NI, C::NCOMP, true>(tab, 0.0, s.q, s.p, s.p, F, qn, pn, qc, pc, qcn, pcn);
 #pragma unroll
             for (int c = 0; c < NI; c++) {
                 s.q[c] = qn[c];
@@ -697,12 +711,19 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
             const double h = t_new - t;
             const double h_try = fabs(h);
 
+            // scaled forces G_l = h^2 F_l and u = h p (dop8_core.cuh dop8_stage_coords): no multiplication by
+            // the trajectory's own h inside the stages
+            const ForceFn<C, true> force_h2{s, h * h};
+            const double hinv = (h < 0.0) ? -fast_rcp(h_try) : fast_rcp(h_try);  // (h = 0: inf; nothing is committed)
+            double u[NI];
+#pragma unroll
+            for (int c = 0; c < NI; c++) u[c] = h * s.p[c];
             double F[12][NI];
-            dop8_stages<NI, false, PAIR>(tab, h, h * h, s.q, s.p, F, force, nohook);
+            dop8_stages<NI, PAIR>(tab, s.q, u, F, force_h2, nohook);
             double qn[NI], pn[NI];
-            dop8_solution<NI, C::NCOMP, false>(tab, h, h * h, s.q, s.p, F, qn, pn, qc, pc, qcn, pcn);
+            dop8_solution<NI, C::NCOMP, false>(tab, hinv, s.q, s.p, u, F, qn, pn, qc, pc, qcn, pcn);
             double S5, S3;
-            dop8_error_sums<NI>(tab, h, s.q, s.p, qn, pn, F, a.rtol, a.atol, on, S5, S3);
+            dop8_error_sums<NI>(tab, hinv, s.q, s.p, qn, pn, F, a.rtol, a.atol, on, S5, S3);
             {
                 double S[2] = {S5, S3};
                 tile_sum_vec<L, 2>(S);
@@ -811,14 +832,14 @@ ld_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const R
     s.load(a.y0, nullptr, a.n_ic, ic, psign);
     if (member > 0) s.displace((member - 1) >> 1, ((member - 1) & 1) ? -a.sigma : a.sigma, psign);
     double M = 0.0;
-    const ForceFn<C> force{s};
+    const ForceFn<C> force{s, 1.0};
     LdHook<C> hook{tab, s, M};
     for (long long st = 0; st < a.n_steps; ++st) {
         double F[12][NI];
-        dop8_stages<NI, true, false>(tab, 0.0, 0.0, s.q, s.p, F, force, hook);
+        dop8_stages<NI, false>(tab, s.q, s.p, F, force, hook);
         double qn[NI], pn[NI];
         double z[1] = {0.0}, zn[1];
-        dop8_solution<NI, 0, true>(tab, 0.0, 0.0, s.q, s.p, F, qn, pn, z, z, zn, zn);
+        dop8_solution<NI, 0, true>(tab, 0.0, s.q, s.p, s.p, F, qn, pn, z, z, zn, zn);
 #pragma unroll
         for (int c = 0; c < NI; c++) {
             s.q[c] = qn[c];

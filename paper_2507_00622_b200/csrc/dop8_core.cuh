@@ -249,33 +249,24 @@ struct LogBank<NV, true> {
 //
 // Stage coordinates of stage i (0-based) from the forces of the earlier stages.  A.A has an EMPTY first
 // subdiagonal ((A.A)_{i,i-1} = 0, pinned by tests/test_library_abi.py): Q_i needs F_0 .. F_{i-2} only.
-template <int I, int NI, bool PREMUL>
-__device__ __forceinline__ void dop8_stage_coords(const Tab& tab, double h, double h2, const double (&q)[NI],
-                                                  const double (&p)[NI], const double (&F)[12][NI],
-                                                  double (&Q)[NI]) {
+// One code path serves both steppers.  Fixed step: `tab` is premultiplied by powers of h (a2 = h^2 A.A,
+// cs = h rowsum(A)), `p` is the momentum, F the forces.  Adaptive step: `tab` is raw, and the caller hands in
+// u = h p in place of p and works with SCALED forces G_l = h^2 F_l (the force functor multiplies by h^2 where
+// that is free): then Q_i = q + cs_i u + sum_l (A.A)_il G_l needs no further
+// multiplication by the trajectory's h, and every fused multiply-add below has a constant-bank coefficient,
+// i.e. at most two register sources (three-register DFMAs run at 2/3 rate).
+template <int I, int NI>
+__device__ __forceinline__ void dop8_stage_coords(const Tab& tab, const double (&q)[NI], const double (&p)[NI],
+                                                  const double (&F)[12][NI], double (&Q)[NI]) {
     static_assert(I >= 1 && I < 12, "stage index");
 #pragma unroll
     for (int c = 0; c < NI; c++) {
-        if constexpr (PREMUL) {
-            double acc = fma(tab.cs[I], p[c], q[c]);
-            static_for<0, I>([&](auto lc) {
-                constexpr int l = decltype(lc)::value;
-                if constexpr (coef::A2[I][l] != 0.0) acc = fma(tab.a2[I][l], F[l][c], acc);
-            });
-            Q[c] = acc;
-        } else {
-            double base = fma(h * tab.cs[I], p[c], q[c]);
-            if constexpr (I == 1) {
-                Q[c] = base;  // row 2 of A.A is empty
-            } else {
-                double s = tab.a2[I][0] * F[0][c];
-                static_for<1, I>([&](auto lc) {
-                    constexpr int l = decltype(lc)::value;
-                    if constexpr (coef::A2[I][l] != 0.0) s = fma(tab.a2[I][l], F[l][c], s);
-                });
-                Q[c] = fma(h2, s, base);
-            }
-        }
+        double acc = fma(tab.cs[I], p[c], q[c]);
+        static_for<0, I>([&](auto lc) {
+            constexpr int l = decltype(lc)::value;
+            if constexpr (coef::A2[I][l] != 0.0) acc = fma(tab.a2[I][l], F[l][c], acc);
+        });
+        Q[c] = acc;
     }
 }
 
@@ -285,20 +276,19 @@ __device__ __forceinline__ void dop8_stage_coords(const Tab& tab, double h, doub
 // scheduler interleaves: twice the instruction-level parallelism exactly where a lane waits on a shuffle
 // and on the short dependent chain of the force.  Same operations in the same order per value: results
 // are bit-identical with PAIR = false.
-template <int NI, bool PREMUL, bool PAIR = true, class Force, class Hook>
-__device__ __forceinline__ void dop8_stages(const Tab& tab, double h, double h2, const double (&q)[NI],
-                                            const double (&p)[NI], double (&F)[12][NI], Force&& force,
-                                            Hook&& hook) {
+template <int NI, bool PAIR = true, class Force, class Hook>
+__device__ __forceinline__ void dop8_stages(const Tab& tab, const double (&q)[NI], const double (&p)[NI],
+                                            double (&F)[12][NI], Force&& force, Hook&& hook) {
     if constexpr (PAIR) {
         static_for<0, 6>([&](auto kc) {
             constexpr int i0 = 2 * decltype(kc)::value, i1 = i0 + 1;
             double Qb[NI];
-            dop8_stage_coords<i1, NI, PREMUL>(tab, h, h2, q, p, F, Qb);
+            dop8_stage_coords<i1, NI>(tab, q, p, F, Qb);
             if constexpr (i0 == 0) {
                 force.pair(q, F[0], Qb, F[i1]);
             } else {
                 double Qa[NI];
-                dop8_stage_coords<i0, NI, PREMUL>(tab, h, h2, q, p, F, Qa);
+                dop8_stage_coords<i0, NI>(tab, q, p, F, Qa);
                 force.pair(Qa, F[i0], Qb, F[i1]);
             }
             hook(Int<i0>{}, F);
@@ -310,7 +300,7 @@ __device__ __forceinline__ void dop8_stages(const Tab& tab, double h, double h2,
         static_for<1, 12>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
             double Q[NI];
-            dop8_stage_coords<i, NI, PREMUL>(tab, h, h2, q, p, F, Q);
+            dop8_stage_coords<i, NI>(tab, q, p, F, Q);
             force(Q, F[i]);
             hook(ic, F);
         });
@@ -321,10 +311,12 @@ __device__ __forceinline__ void dop8_stages(const Tab& tab, double h, double h2,
 // with a compensated sum: y+ = y + (dy + c) by Fast2Sum, the rounding
 // error of that one addition -- which is ~1/h times larger than every other rounding error of a
 // step -- is carried in c to the next step.  qc/pc: carried words in, qcn/pcn: out.
+// PREMUL (fixed step): premultiplied table, F = forces.  Otherwise (adaptive): raw table, u = h p,
+// F = the scaled forces h^2 F_l, hinv = 1/h:  q+ = q + u + sum bq_l G_l,  p+ = p + hinv sum b_l G_l.
 template <int NI, int NCOMP, bool PREMUL>
-__device__ __forceinline__ void dop8_solution(const Tab& tab, double h, double h2, const double (&q)[NI],
-                                              const double (&p)[NI], const double (&F)[12][NI],
-                                              double (&qn)[NI], double (&pn)[NI],
+__device__ __forceinline__ void dop8_solution(const Tab& tab, double hinv, const double (&q)[NI],
+                                              const double (&p)[NI], const double (&u)[NI],
+                                              const double (&F)[12][NI], double (&qn)[NI], double (&pn)[NI],
                                               const double (&qc)[NCOMP > 0 ? NCOMP : 1],
                                               const double (&pc)[NCOMP > 0 ? NCOMP : 1],
                                               double (&qcn)[NCOMP > 0 ? NCOMP : 1],
@@ -342,15 +334,14 @@ __device__ __forceinline__ void dop8_solution(const Tab& tab, double h, double h
                 if constexpr (coef::B[l] != 0.0) ap = fma(tab.bp[l], F[l][c], ap);
             });
         } else {
-            double sq = tab.bq[0] * F[0][c];
+            aq = comp ? u[c] + qc[comp ? c : 0] : u[c] + q[c];
             double sp = tab.bp[0] * F[0][c];
-            static_for<1, 12>([&](auto lc) {
+            static_for<0, 12>([&](auto lc) {
                 constexpr int l = decltype(lc)::value;
-                if constexpr (coef::BQ[l] != 0.0) sq = fma(tab.bq[l], F[l][c], sq);
-                if constexpr (coef::B[l] != 0.0) sp = fma(tab.bp[l], F[l][c], sp);
+                if constexpr (coef::BQ[l] != 0.0) aq = fma(tab.bq[l], F[l][c], aq);
+                if constexpr (l > 0 && coef::B[l] != 0.0) sp = fma(tab.bp[l], F[l][c], sp);
             });
-            aq = comp ? fma(h2, sq, fma(h, p[c], qc[comp ? c : 0])) : fma(h2, sq, fma(h, p[c], q[c]));
-            ap = comp ? fma(h, sp, pc[comp ? c : 0]) : fma(h, sp, p[c]);
+            ap = comp ? fma(hinv, sp, pc[comp ? c : 0]) : fma(hinv, sp, p[c]);
         }
         if (comp) {  // aq, ap are increments (+ carried error): Fast2Sum
             const double tq = q[c] + aq, tp = p[c] + ap;
@@ -367,14 +358,16 @@ __device__ __forceinline__ void dop8_solution(const Tab& tab, double h, double h
 
 // Embedded error sums of one attempted step:
 // this lane's contribution to S5 = sum_c (e5_c/scale_c)^2 and S3 likewise, over its 2 NI
-// components, scale_c = atol + rtol max(|y_c|, |y+_c|).  Raw tableau (h applied here).
-// `on[c]` masks padding items.
+// components, scale_c = atol + rtol max(|y_c|, |y+_c|).  Raw tableau, F = the SCALED forces h^2 F_l:
+// the sums are of (e_c / h) / scale_c (the controller multiplies the norm by |h| afterwards), i.e.
+// e_q / h = hinv sum (E^T A)_l G_l,  e_p / h = hinv^2 sum E_l G_l.  `on[c]` masks padding items.
 template <int NI>
-__device__ __forceinline__ void dop8_error_sums(const Tab& tab, double h, const double (&q)[NI],
+__device__ __forceinline__ void dop8_error_sums(const Tab& tab, double hinv, const double (&q)[NI],
                                                 const double (&p)[NI], const double (&qn)[NI],
                                                 const double (&pn)[NI], const double (&F)[12][NI],
                                                 double rtol, double atol, const bool (&on)[NI], double& S5,
                                                 double& S3) {
+    const double hinv2 = hinv * hinv;
     // NACC interleaved partial sums (items c, c + NACC, ... go to sum c % NACC): the dependent chain is
     // 2 NI / NACC fused multiply-adds deep instead of 2 NI (the error norm is on the serial tail of an attempt)
     constexpr int NACC = NI < 3 ? NI : 3;
@@ -390,9 +383,9 @@ __device__ __forceinline__ void dop8_error_sums(const Tab& tab, double h, const 
             if constexpr (coef::E5[l] != 0.0) s5p = fma(tab.e5p[l], F[l][c], s5p);
             if constexpr (coef::E3[l] != 0.0) s3p = fma(tab.e3p[l], F[l][c], s3p);
         });
-        double iq = fast_rcp(fma(rtol, fmax(fabs(q[c]), fabs(qn[c])), atol));
-        double ip = fast_rcp(fma(rtol, fmax(fabs(p[c]), fabs(pn[c])), atol));
-        double a = h * s5q * iq, b = s5p * ip, c3 = h * s3q * iq, d3 = s3p * ip;
+        const double iq = hinv * fast_rcp(fma(rtol, fmax(fabs(q[c]), fabs(qn[c])), atol));
+        const double ip = hinv2 * fast_rcp(fma(rtol, fmax(fabs(p[c]), fabs(pn[c])), atol));
+        const double a = s5q * iq, b = s5p * ip, c3 = s3q * iq, d3 = s3p * ip;
         if (c < NACC) {
             a5[c % NACC] = on[c] ? fma(a, a, b * b) : 0.0;
             a3[c % NACC] = on[c] ? fma(c3, c3, d3 * d3) : 0.0;

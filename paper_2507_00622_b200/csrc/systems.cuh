@@ -5,8 +5,10 @@
 //
 // Interface used by the column layout (col_kernels.cuh), NDOF coordinates per column:
 //   force(prm, Q, F)          F = -grad V(Q)                        (orbit column)
-//   hess(prm, Q, s)           the entries of  M(s) = V2'' + s V3''(Q)
-//   apply(H, x, G)            G = -M x
+//   hess(prm, Q, s, g)        the entries of  g M(s),  M(s) = V2'' + s V3''(Q)   (g = 1, or h^2 where the
+//                             adaptive kernels want scaled forces: dop8_core.cuh dop8_stage_coords)
+//   apply(H, x, G)            G = -H x
+//   force_hess(prm, H, Q, g, F)  F = -g grad V(Q) for the orbit, reusing H = g M(1) (the same row products)
 // For these cubic potentials  grad V(Q) = (V2'' + 1/2 V3''(Q)) Q  (Euler's relation for the
 // homogeneous cubic part), so an orbit column can also be advanced branch-free as
 // apply(hess(Q, 1/2), Q): that is what a lane does when orbit and deviation columns sit on
@@ -27,9 +29,15 @@ struct HenonHeiles {
         F[1] = fma(y, y, -y) - x * x;     // py' = -y - x^2 + y^2
     }
     // V_qq = [[1+2y, 2x],[2x, 1-2y]]
-    __device__ static __forceinline__ Hess hess(const Params&, const double* Q, double s) {
-        const double tx = 2.0 * s * Q[0], ty = 2.0 * s * Q[1];
-        return Hess{1.0 + ty, tx, 1.0 - ty};
+    __device__ static __forceinline__ Hess hess(const Params&, const double* Q, double s, double g = 1.0) {
+        const double t = 2.0 * s * g;
+        return Hess{fma(t, Q[1], g), t * Q[0], fma(-t, Q[1], g)};
+    }
+    // -g grad V = -g (x (1 + 2y), y - y^2 + x^2) with H = g M(1): the first row is H.xx x
+    __device__ static __forceinline__ void force_hess(const Params&, const Hess& H, const double* Q, double g, double* F) {
+        const double x = Q[0], y = Q[1];
+        F[0] = -(H.xx * x);
+        F[1] = g * fma(-x, x, fma(y, y, -y));
     }
     __device__ static __forceinline__ void apply(const Hess& H, const double* x, double* G) {
         G[0] = -fma(H.xx, x[0], H.xy * x[1]);
@@ -64,9 +72,15 @@ struct Coupled3 {
         F[2] = -P.w3s * q3 - P.e * q2 * q2;
     }
     // V_qq = [[w1^2+2e q2, 2e q1, 0],[2e q1, w2^2+2e q3, 2e q2],[0, 2e q2, w3^2]]
-    __device__ static __forceinline__ Hess hess(const Params& P, const double* Q, double s) {
-        const double te = 2.0 * P.e * s;
-        return Hess{fma(te, Q[1], P.w1s), te * Q[0], fma(te, Q[2], P.w2s), te * Q[1], P.w3s};
+    __device__ static __forceinline__ Hess hess(const Params& P, const double* Q, double s, double g = 1.0) {
+        const double te = 2.0 * P.e * s * g;
+        return Hess{fma(te, Q[1], g * P.w1s), te * Q[0], fma(te, Q[2], g * P.w2s), te * Q[1], g * P.w3s};
+    }
+    // -g grad V with H = g M(1): h12 = 2 g e q1 and h23 = 2 g e q2 carry the quadratic terms, halved
+    __device__ static __forceinline__ void force_hess(const Params&, const Hess& H, const double* Q, double, double* F) {
+        F[0] = -(H.h11 * Q[0]);
+        F[1] = -fma(H.h22, Q[1], 0.5 * H.h12 * Q[0]);
+        F[2] = -fma(H.h33, Q[2], 0.5 * H.h23 * Q[1]);
     }
     __device__ static __forceinline__ void apply(const Hess& H, const double* x, double* G) {
         G[0] = -fma(H.h11, x[0], H.h12 * x[1]);
