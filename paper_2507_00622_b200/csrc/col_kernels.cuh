@@ -654,15 +654,41 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
         // without it, exactly one trajectory per tile.  The warp-wide loop and every section that
         // shuffles stay convergent; per-tile decisions are predicates.
         const double dir = (a.t_end >= a.t0) ? 1.0 : -1.0;
+        const bool fwd = dir > 0.0;
         const double interval = fabs(a.t_end - a.t0);
         bool on[NI];
         s.on_mask(on);
         double h_abs = 0.0, min_step = 0.0;
         long long attempts = 0, ic = 0;
-        bool rejected = false, need = true, done = false, first_fetch = true;
+        bool rejected = false, need = true, fin = false, done = false, first_fetch = true;
+        bool more = false;  // t has not reached t_end yet
         int cd = a.m;
+        // One vote per iteration: the block below (write out the trajectories that ended in the previous
+        // attempt, fetch new ones, leave when nothing is left) is entered only when some tile asks for it.
         while (true) {
-            if (group_any<L>(need)) {
+            if (group_any<L>(fin || need)) {
+                if (group_any<L>(fin)) {
+                    bool bad = !s.finite_all();
+                    bad = tile_any<L>(status != ST_OK) || bad;
+                    double ind = 0.0;
+                    if constexpr (IND != IND_NONE) ind = s.template indicator<IND>();
+                    if (fin) {
+                        const int st_out = (bad && status == ST_OK) ? (int)ST_NONFINITE : status;
+                        s.store(a.y, a.w, a.n_ic, ic, bad);
+                        if constexpr (K > 0) s.store_logs(a, ic, bad, t - a.t0);
+                        if (s.lt == 0) {
+                            if constexpr (IND != IND_NONE) {
+                                if (a.series) a.series[ic] = bad ? nan("") : ind;  // adaptive: n_samples = 1
+                            }
+                            if (a.n_acc) a.n_acc[ic] = n_acc;
+                            if (a.n_rej) a.n_rej[ic] = n_rej;
+                            if (a.status) a.status[ic] = st_out;
+                            if (a.t_final) a.t_final[ic] = t;
+                        }
+                        need = true;
+                        fin = false;
+                    }
+                }
                 long long nxt = a.n_ic;  // "nothing left"
                 if (a.queue != nullptr) {
                     if (need && s.lt == 0) nxt = (long long)atomicAdd(a.queue, 1ULL);
@@ -678,6 +704,7 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
                     s.load(a.y, a.w, a.n_ic, ic, 1.0);
                     s.reset_logs();
                     t = a.t0;
+                    more = interval > 0.0;
                     n_acc = n_rej = attempts = 0;
                     status = ST_OK;
                     rejected = false;
@@ -689,37 +716,37 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
                 const double h_init = a.h0 > 0.0 ? a.h0 : initial_step(s, interval, dir, a.rtol, a.atol);
                 if (got) h_abs = h_init;
                 need = false;
+                if (!group_any<L>(!done)) break;
             }
-            if (!group_any<L>(!done)) break;
 
-            bool active = !done && status == ST_OK && dir * (a.t_end - t) > 0.0;
-            if (!rejected) {
-                min_step = ten_ulp(t, dir);  // 10 |nextafter(t, dir inf) - t|
-                h_abs = fmax(h_abs, min_step);
+            // ---- one attempt; everything below is selects, no branch (one basic block for the scheduler) ----
+            bool active = !done && status == ST_OK && more;
+            {
+                const double ms = ten_ulp(t, dir);  // 10 |nextafter(t, dir inf) - t|
+                min_step = rejected ? min_step : ms;
+                h_abs = rejected ? h_abs : fmax(h_abs, ms);
             }
-            if (active && h_abs < min_step) {
-                status = ST_UNDERFLOW;
-                active = false;
-            }
-            if (active && a.max_steps > 0 && attempts >= a.max_steps) {
-                status = ST_MAXSTEPS;
-                active = false;
-            }
+            const bool under = active && h_abs < min_step;
+            status = under ? (int)ST_UNDERFLOW : status;
+            active = active && !under;
+            const bool maxed = active && a.max_steps > 0 && attempts >= a.max_steps;
+            status = maxed ? (int)ST_MAXSTEPS : status;
+            active = active && !maxed;
             attempts += active ? 1 : 0;
             double t_new = t + h_abs * dir;
-            if (dir * (t_new - a.t_end) > 0.0) t_new = a.t_end;  // land exactly on t_end
+            if (fwd ? (t_new > a.t_end) : (t_new < a.t_end)) t_new = a.t_end;  // land exactly on t_end
             const double h = t_new - t;
             const double h_try = fabs(h);
 
             // scaled forces G_l = h^2 F_l and u = h p (dop8_core.cuh dop8_stage_coords): no multiplication by
             // the trajectory's own h inside the stages
             const ForceFn<C, true> force_h2{s, h * h};
-            const double hinv = (h < 0.0) ? -fast_rcp(h_try) : fast_rcp(h_try);  // (h = 0: inf; nothing is committed)
             double u[NI];
 #pragma unroll
             for (int c = 0; c < NI; c++) u[c] = h * s.p[c];
             double F[12][NI];
             dop8_stages<NI, PAIR>(tab, s.q, u, F, force_h2, nohook);
+            const double hinv = fwd ? fast_rcp(h_try) : -fast_rcp(h_try);  // (h = 0: inf; nothing is committed)
             double qn[NI], pn[NI];
             dop8_solution<NI, C::NCOMP, false>(tab, hinv, s.q, s.p, u, F, qn, pn, qc, pc, qcn, pcn);
             double S5, S3;
@@ -731,9 +758,7 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
                 S3 = S[1];
             }
             // err = |h| S5 / sqrt(D (S5 + 0.01 S3)) against 1, and the step-size factor 0.9 err^(-1/8), without
-            // forming err (dop8_core.cuh "step-size controller"): accept <=> num^2 < den.  The whole decision is
-            // written with selects, not branches: one basic block, so the short controller chain, the commit and
-            // (thread layout) the renormalisation of the new vectors are scheduled side by side.
+            // forming err (dop8_core.cuh "step-size controller"): accept <=> num^2 < den
             const double num = h_try * S5, den = fma(0.01, S3, S5) * s.dcount(), num2 = num * num;
             const bool zero = (S5 == 0.0) && (S3 == 0.0);          // err = 0
             const bool acc = active && (zero || num2 < den);
@@ -749,6 +774,7 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
             n_acc += acc ? 1 : 0;
             n_rej += rej ? 1 : 0;
             t = acc ? t_new : t;
+            more = fwd ? (t < a.t_end) : (t > a.t_end);
 #pragma unroll
             for (int c = 0; c < NI; c++) {
                 s.q[c] = acc ? qn[c] : s.q[c];
@@ -759,14 +785,11 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
                 qc[c] = acc ? qcn[c] : qc[c];
                 pc[c] = acc ? pcn[c] : pc[c];
             }
-            bool ren = false;
             if constexpr (MODE != MODE_NONE) {
-                if (acc) {
-                    const bool at_end = !(dir * (a.t_end - t) > 0.0);
-                    if (--cd == 0 || at_end) {
-                        cd = a.m;
-                        ren = true;
-                    }
+                bool ren = false;
+                if (acc && (--cd == 0 || !more)) {
+                    cd = a.m;
+                    ren = true;
                 }
                 // thread layout: renormalising is lane-local and cheap, so it runs every attempt under the
                 // predicate (no branch between it and the controller); tiles shuffle: only when some tile wants it
@@ -776,30 +799,8 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
                     if (ren) s.scrub_carry(qc, pc);
                 }
             }
-
-            // trajectories that ended in this iteration: write their results, ask for the next one
-            const bool fin = !done && !(status == ST_OK && dir * (a.t_end - t) > 0.0);
-            if (group_any<L>(fin)) {
-                bool bad = !s.finite_all();
-                bad = tile_any<L>(status != ST_OK) || bad;
-                double ind = 0.0;
-                if constexpr (IND != IND_NONE) ind = s.template indicator<IND>();
-                if (fin) {
-                    const int st_out = (bad && status == ST_OK) ? (int)ST_NONFINITE : status;
-                    s.store(a.y, a.w, a.n_ic, ic, bad);
-                    if constexpr (K > 0) s.store_logs(a, ic, bad, t - a.t0);
-                    if (s.lt == 0) {
-                        if constexpr (IND != IND_NONE) {
-                            if (a.series) a.series[ic] = bad ? nan("") : ind;  // adaptive: n_samples = 1
-                        }
-                        if (a.n_acc) a.n_acc[ic] = n_acc;
-                        if (a.n_rej) a.n_rej[ic] = n_rej;
-                        if (a.status) a.status[ic] = st_out;
-                        if (a.t_final) a.t_final[ic] = t;
-                    }
-                    need = true;
-                }
-            }
+            // trajectories that ended in this attempt: written out at the top of the next iteration
+            fin = !done && !(status == ST_OK && more);
         }
     }
 }

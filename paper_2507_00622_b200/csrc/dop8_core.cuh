@@ -172,7 +172,6 @@ __device__ __forceinline__ double fast_rcp(double x) {
     const double e = fma(-x, r0, 1.0);
     return fma(r0, fma(e, fma(e, e, e), e), r0);
 }
-
 // ---- deferred logarithm ----------------------------------------------------------------------
 // sum_k ln(r_k) of the renormalisation factors is kept as a running PRODUCT in
 // (mantissa in [1,2), integer exponent) form: one DMUL and a few integer instructions per factor
@@ -436,18 +435,21 @@ __device__ __forceinline__ float step_factor(double num2, double den) {  // 0.9 
 }
 
 // 10 |nextafter(t, dir inf) - t|: the smallest step the controller allows at time t (DESIGN.md "Adaptive
-// step", item 5).  The spacing of the doubles at t is 2^(e - 1075) (e: biased exponent), half of that when
-// t is a power of two and the step points towards zero; 10 x 2^k = 1.25 x 2^(k+3) is assembled from integer
-// instructions -- exact, and nothing on the FP64 pipe.  t = 0, subnormal or tiny t (result would be
-// subnormal), inf and NaN take the library route.
+// step", item 5), assembled from integer instructions: exact, branch-free, nothing on the FP64 pipe.  The
+// spacing of the doubles at t is 2^(e - 1075) (e: biased exponent of t, at least 1), half of that when t is a
+// power of two and the step points towards zero.  Where 10 x spacing is a normal number (e >= 50) it is
+// 1.25 x 2^(k+3) -- exponent field k + 1026, mantissa 0x4000000000000; below that it is subnormal, i.e. the
+// integer 10 << (e - 1) in units of 2^-1074 (t = 0: 10 x 4.9e-324, as nextafter gives).
 __device__ __forceinline__ double ten_ulp(double t, double dir) {
     const int hi = __double2hiint(t), lo = __double2loint(t);
     const int e = (hi >> 20) & 0x7ff;
     const bool pow2 = ((hi & 0xfffff) | lo) == 0;
     const bool to_zero = (hi < 0) == (dir > 0.0);  // sign(t) opposite to the direction of integration
-    const int ef = e - 1075 + 3 + 1023 - ((pow2 && to_zero) ? 1 : 0);
-    if (e < 64 || e == 0x7ff) return 10.0 * fabs(nextafter(t, dir * INFINITY) - t);
-    return __hiloint2double((ef << 20) | 0x40000, 0);
+    const int adj = (pow2 && to_zero && e > 1) ? 1 : 0;
+    const double normal = __hiloint2double(((e - 49 - adj) << 20) | 0x40000, 0);
+    const int sh = (e > 0 ? e - 1 : 0) - adj;
+    const double tiny = __longlong_as_double(10LL << (sh & 63));
+    return (e - adj) >= 50 ? normal : tiny;
 }
 
 }  // namespace chs

@@ -8,7 +8,7 @@ int try_launch_hh_adapt(const LaunchReq& rq) {
         if (rq.args.n_ic <= 4096) return run_col<HenonHeiles, 2, 4, MODE_NORM, IND_SALI, true, 128, 3>(rq);
         return run_col<HenonHeiles, 2, 1, MODE_NORM, IND_SALI, true, 128, 1>(rq);
     }
-    if (CHS_MATCH(0, WHAT_GALI, 2, 1)) return run_col<HenonHeiles, 2, 1, MODE_NORM, IND_GALI, true, 128, 1>(rq);
+    if (CHS_MATCH(0, WHAT_GALI, 2, 1)) return run_col<HenonHeiles, 2, 4, MODE_NORM, IND_GALI, true, 128, 3>(rq);  // (one thread per trajectory would spill)
     if (CHS_MATCH(0, WHAT_LYAP, 1, 1)) return run_col<HenonHeiles, 1, 1, MODE_MGS, IND_NONE, true, 128, 2>(rq);
     if (CHS_MATCH(0, WHAT_LYAP, 2, 1)) return run_col<HenonHeiles, 2, 1, MODE_MGS, IND_NONE, true, 128, 1>(rq);
     return -1;
