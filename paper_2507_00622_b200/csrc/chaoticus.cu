@@ -4,7 +4,6 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
-#include <cstdlib>
 
 #include "../../include/chaoticus.h"
 #include "launch.h"
@@ -248,7 +247,6 @@ int run_common(int what, const chs_problem* pb, long long n_ic, double* y, doubl
     rq.tab = make_tab(st->adaptive ? 1.0 : st->h);
     rq.stream = (cudaStream_t)stream;
     rq.info = info;
-    { const char* tv = getenv("CHS_TUNE"); rq.tune = tv ? atoi(tv) : 0; }  // DEV KNOB
     chs::RunArgs& a = rq.args;
     a.n_ic = n_ic;
     a.y = y;

@@ -303,11 +303,14 @@ struct Col {
 #pragma unroll
         for (int j = 0; j < CPL; j++) {
             if (L == 1 && j == 0) continue;  // the orbit
-            double s = 0.0;
+            double sd[ND];  // per-coordinate q^2 + p^2, then a short sum: 2 + log2(ND) levels deep, not 2 ND
 #pragma unroll
-            for (int d = 0; d < ND; d++) s = fma(q[j * ND + d], q[j * ND + d], fma(p[j * ND + d], p[j * ND + d], s));
+            for (int d = 0; d < ND; d++) sd[d] = fma(q[j * ND + d], q[j * ND + d], p[j * ND + d] * p[j * ND + d]);
+            double s = sd[0];
+#pragma unroll
+            for (int d = 1; d < ND; d++) s += sd[d];
             const bool dev = is_dev(j) && apply;
-            const double ri = fast_rsqrt(s);
+            const double ri = fast_rsqrt_short(s);
             const double inv = dev ? ri : 1.0;
 #pragma unroll
             for (int d = 0; d < ND; d++) {

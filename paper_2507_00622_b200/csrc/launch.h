@@ -23,7 +23,6 @@ struct LaunchReq {
     KernelInfo* info;  // non-null: report the launch shape, launch nothing
     // LD: which directions
     int dir_first, n_dirs;
-    int tune;  // DEV KNOB (env CHS_TUNE) -- remove before the round ends
 };
 
 // each returns -1 if it has no kernel for the request, else a cudaError_t (0 = success)
