@@ -310,7 +310,7 @@ struct Col {
 #pragma unroll
             for (int d = 1; d < ND; d++) s += sd[d];
             const bool dev = is_dev(j) && apply;
-            const double ri = fast_rsqrt_short(s);
+            const double ri = fast_rsqrt(s);
             const double inv = dev ? ri : 1.0;
 #pragma unroll
             for (int d = 0; d < ND; d++) {

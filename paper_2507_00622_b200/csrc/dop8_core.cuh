@@ -137,11 +137,11 @@ __device__ __forceinline__ bool group_any(bool b) {
 }
 
 // ---- square roots off the slow path ----------------------------------------------------------
-// MUFU.RSQ64H seed y0 (|1 - x y0^2| <= 2^-19, measured) and the cubic Taylor polynomial of
-// (1-e)^(-1/2): relative error <= 1 ulp (measured against sqrt() over 1.6e8 arguments), 6 FP64
-// instructions none of which reads three distinct registers (those run at
-// 2/3 rate), no branch.  The library sqrt()/1.0/sqrt() cost 8 + ~10 instructions and a slow-path
-// branch.  Arguments are sums of squares: x >= 0.
+// MUFU.RSQ64H seed y0 (|1 - x y0^2| = |e| <= 2^-19, measured) and the quadratic Taylor polynomial of
+// (1-e)^(-1/2) = 1 + e/2 + 3e^2/8 + (5/16 e^3 <= 2^-59: below half an ulp, dropped): 5 FP64 instructions none of
+// which reads three distinct registers (those run at 2/3 rate), 4 dependent levels after
+// the seed, no branch.  The library sqrt()/1.0/sqrt() cost 8 + ~10 instructions and a slow-path branch.
+// Arguments are sums of squares: x >= 0.
 __device__ __forceinline__ double rsqrt_seed(double x) {
     double y;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
@@ -151,15 +151,6 @@ __device__ __forceinline__ double rsqrt_seed(double x) {
 __device__ __forceinline__ double fast_rsqrt(double x) {
     const double y0 = rsqrt_seed(x);
     const double e = fma(-(x * y0), y0, 1.0);
-    const double t = fma(e, fma(e, 0.3125, 0.375), 0.5);
-    return fma(y0, e * t, y0);
-}
-// the same value with a shorter dependent chain (4 levels after the seed instead of 6) for the renormalisation
-// of latency-bound small ensembles: y0 (1 + e/2 + 3 e^2/8) as fma(y0 e, fma(e, 3/8, 1/2), y0); the dropped cubic
-// term is 0.3125 e^3 <= 2^-58.
-__device__ __forceinline__ double fast_rsqrt_short(double x) {
-    const double y0 = rsqrt_seed(x);
-    const double e = fma(-(x * y0), y0, 1.0);
     return fma(y0 * e, fma(e, 0.375, 0.5), y0);
 }
 // sqrt(x); x = 0 (or denormal) gives 0
@@ -167,8 +158,7 @@ __device__ __forceinline__ double fast_sqrt(double x) {
     const double y0 = rsqrt_seed(x);
     const double g0 = x * y0;
     const double e = fma(-g0, y0, 1.0);
-    const double t = fma(e, fma(e, 0.3125, 0.375), 0.5);
-    const double r = fma(g0, e * t, g0);
+    const double r = fma(g0 * e, fma(e, 0.375, 0.5), g0);
     return (__double2hiint(x) < 0x00100000) ? 0.0 : r;  // integer test: stays off the FP64 pipe
 }
 
