@@ -762,17 +762,10 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
             }
             // err = |h| S5 / sqrt(D (S5 + 0.01 S3)) against 1, and the step-size factor 0.9 err^(-1/8), without
             // forming err (dop8_core.cuh "step-size controller"): accept <=> num^2 < den
-            const double num = h_try * S5, den = fma(0.01, S3, S5) * s.dcount(), num2 = num * num;
-            const bool zero = (S5 == 0.0) && (S3 == 0.0);          // err = 0
-            const bool acc = active && (zero || num2 < den);
-            const bool rej = active && !zero && num2 >= den;
-            if (active && !acc && !rej) status = ST_NONFINITE;       // NaN: inf or NaN in y+ (fast_rcp(inf) is NaN)
-            const float ff = step_factor(num2, den);
-            const double fd = (double)ff;
-            const float cap = rejected ? 1.0f : 10.0f;               // <= 1 right after a rejection
-            const double f_acc = (zero || !(ff < cap)) ? (double)cap : fd;
-            const double f_rej = (ff > 0.2f) ? fd : 0.2;
-            if (acc || rej) h_abs = h_try * (acc ? f_acc : f_rej);
+            const StepDecision dec = step_decision(h_try, S5, S3, s.dcount(), rejected);
+            const bool acc = active && dec.acc, rej = active && dec.rej;
+            if (active && !acc && !rej) status = ST_NONFINITE;  // NaN: inf or NaN in y+ (fast_rcp(inf) is NaN)
+            if (acc || rej) h_abs = h_try * dec.factor;
             rejected = rej ? true : (acc ? false : rejected);
             n_acc += acc ? 1 : 0;
             n_rej += rej ? 1 : 0;

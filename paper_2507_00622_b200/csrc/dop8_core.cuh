@@ -405,8 +405,6 @@ enum : int { ST_OK = 0, ST_NONFINITE = 1, ST_UNDERFLOW = 2, ST_MAXSTEPS = 3 };
 
 // x^(1/8) by three square roots (the starting step's exponent)
 __device__ __forceinline__ double root8(double x) { return sqrt(sqrt(sqrt(x))); }
-// x^(-1/8), x > 0 finite: branch-free (the generic first-order kernels' controller, gen_kernels.cuh)
-__device__ __forceinline__ double inv_root8(double x) { return fast_rsqrt(fast_sqrt(fast_sqrt(x))); }
 
 // ---- the step-size controller off the FP64 critical path ("Serial tail") ----
 // With num = |h| S5 and den = D (S5 + 0.01 S3) the error norm is err = num / sqrt(den), so
@@ -430,6 +428,30 @@ __device__ __forceinline__ float step_factor(double num2, double den) {  // 0.9 
     float f;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(f) : "f"(e));
     return f;
+}
+
+// The decision of one attempt (items 3-4), shared by every adaptive kernel.
+// S5, S3: the error sums over all D components; h_try = |h|; rejected: the previous attempt of this step was
+// rejected.  acc / rej: accepted / rejected (neither: S5 or S3 is NaN -- a non-finite y+); factor: what the
+// next |h| is h_try times (accept: min(10, 0.9 err^(-1/8)), at most 1 right after a rejection, 10 when
+// err = 0; reject: max(0.2, 0.9 err^(-1/8))).  Selects only, no branch.
+struct StepDecision {
+    bool acc, rej;
+    double factor;
+};
+__device__ __forceinline__ StepDecision step_decision(double h_try, double S5, double S3, double D, bool rejected) {
+    const double num = h_try * S5, den = fma(0.01, S3, S5) * D, num2 = num * num;
+    const bool zero = (S5 == 0.0) && (S3 == 0.0);  // err = 0
+    StepDecision d;
+    d.acc = zero || num2 < den;
+    d.rej = !zero && num2 >= den;
+    const float ff = step_factor(num2, den);
+    const double fd = (double)ff;
+    const float cap = rejected ? 1.0f : 10.0f;
+    const double f_acc = (zero || !(ff < cap)) ? (double)cap : fd;
+    const double f_rej = (ff > 0.2f) ? fd : 0.2;
+    d.factor = d.acc ? f_acc : f_rej;
+    return d;
 }
 
 // 10 |nextafter(t, dir inf) - t|: the smallest step the controller allows at time t (DESIGN.md "Adaptive

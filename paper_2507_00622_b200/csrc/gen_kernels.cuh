@@ -216,7 +216,7 @@ gen_run_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, 
         double min_step = 0.0;
         while (status == ST_OK && dir * (a.t_end - t) > 0.0) {
             if (!rejected) {
-                min_step = 10.0 * fabs(nextafter(t, dir * INFINITY) - t);
+                min_step = ten_ulp(t, dir);  // 10 |nextafter(t, dir inf) - t|
                 h_abs = fmax(h_abs, min_step);
             }
             if (h_abs < min_step) { status = ST_UNDERFLOW; break; }
@@ -250,11 +250,9 @@ gen_run_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, 
                 S5 = fma(u, u, S5);
                 S3 = fma(v, v, S3);
             }
-            const double err = (S5 == 0.0 && S3 == 0.0) ? 0.0 : h_try * S5 * fast_rsqrt((S5 + 0.01 * S3) * (double)N);
-            if (err < 1.0) {
-                double factor = (err == 0.0) ? 10.0 : fmin(10.0, 0.9 * inv_root8(err));
-                if (rejected) factor = fmin(factor, 1.0);
-                h_abs = h_try * factor;
+            const StepDecision dec = step_decision(h_try, S5, S3, (double)N, rejected);
+            if (dec.acc) {
+                h_abs = h_try * dec.factor;
                 t = t_new;
                 bool fin = true;
 #pragma unroll
@@ -266,8 +264,8 @@ gen_run_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, 
                 n_acc++;
                 rejected = false;
                 if (!fin) status = ST_NONFINITE;
-            } else if (err >= 1.0) {
-                h_abs = h_try * fmax(0.2, 0.9 * inv_root8(err));
+            } else if (dec.rej) {
+                h_abs = h_try * dec.factor;
                 rejected = true;
                 n_rej++;
             } else {
@@ -526,7 +524,7 @@ gen_col_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, 
             bool active = status == ST_OK && dir * (a.t_end - t) > 0.0;
             if (!__any_sync(0xffffffffu, active)) break;
             if (!rejected) {
-                min_step = 10.0 * fabs(nextafter(t, dir * INFINITY) - t);
+                min_step = ten_ulp(t, dir);  // 10 |nextafter(t, dir inf) - t|
                 h_abs = fmax(h_abs, min_step);
             }
             if (active && h_abs < min_step) { status = ST_UNDERFLOW; active = false; }
@@ -567,13 +565,11 @@ gen_col_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, 
             }
             S5 = tile_sum<L>(S5);
             S3 = tile_sum<L>(S3);
-            const double err = (S5 == 0.0 && S3 == 0.0) ? 0.0 : h_try * S5 * fast_rsqrt((S5 + 0.01 * S3) * D);
+            const StepDecision dec = step_decision(h_try, S5, S3, D, rejected);
             bool ren = false;
             if (active) {
-                if (err < 1.0) {
-                    double factor = (err == 0.0) ? 10.0 : fmin(10.0, 0.9 * inv_root8(err));
-                    if (rejected) factor = fmin(factor, 1.0);
-                    h_abs = h_try * factor;
+                if (dec.acc) {
+                    h_abs = h_try * dec.factor;
                     t = t_new;
                     commit(yn, ycn);
                     n_acc++;
@@ -583,8 +579,8 @@ gen_col_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, 
                         cd = a.m;
                         ren = true;
                     }
-                } else if (err >= 1.0) {
-                    h_abs = h_try * fmax(0.2, 0.9 * inv_root8(err));
+                } else if (dec.rej) {
+                    h_abs = h_try * dec.factor;
                     rejected = true;
                     n_rej++;
                 } else {
