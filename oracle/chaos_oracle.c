@@ -74,6 +74,7 @@ typedef struct {
     const double *params;
     int n; /* phase-space dimension 2N, ordering y = (q_1..q_N, p_1..p_N) */
     int k; /* number of deviation vectors */
+    int ld; /* 1: the state carries one more component M with M' = |f(y)|_2 (adaptive Lagrangian descriptor) */
 } prob_t;
 
 int orc_real_bytes(void) { return (int)sizeof(real); }
@@ -330,6 +331,13 @@ static void rhs_aug(const prob_t *pb, const real *Y, real *F)
         dp_orbit(pb->params, Y, F);
         for (int v = 1; v <= pb->k; v++) dp_dev(pb->params, Y, Y + v * n, F + v * n);
         break;
+    }
+    /* PAPER.md:39 "the Lagrangian Descriptor must be calculated alongside the trajectory's evolution":
+     * the arc-length descriptor as one more component of the ODE, M' = |f(y)|_2 (R12, R21) */
+    if (pb->ld) {
+        real s2 = 0;
+        for (int c = 0; c < n; c++) s2 += F[c] * F[c];
+        F[n * (1 + pb->k)] = R_SQRT(s2);
     }
 }
 
@@ -594,7 +602,7 @@ static void run_traj(const prob_t *pb, real *Y, const stepper_t *st, int mode, i
                      int sample_every, long long n_samples, double *series, long long series_stride,
                      real *L, report_t *rep, work_t *wk)
 {
-    int D = pb->n * (1 + pb->k);
+    int D = pb->n * (1 + pb->k) + pb->ld;
     long long n_renorm = 0, slot = 0;
     rep->n_acc = rep->n_rej = 0;
     rep->status = ST_OK;
@@ -865,6 +873,53 @@ int orc_ld_neighbours(int sys, const double *params, long long n_ic, const doubl
 /* ------------------------------------------------------------------------------------
  * Small single-trajectory entry points used only by the pins.
  * ---------------------------------------------------------------------------------- */
+
+/* Lagrangian descriptor with the ADAPTIVE solver ("DOP 8(5) ODE solver with adaptive step size",
+ * PAPER.md:39 the descriptor "calculated alongside the trajectory's evolution"; R21): the
+ * augmented ODE (y, M), M' = |f(y)|_2, M(t0) = 0, through the same adaptive stepper as every other run --
+ * M is one more component of the state, so it takes part in the error norm (D = n + 1) like any other.
+ * Forward: t0 -> t0 + tau, ld_fwd = M.  Backward: t0 -> t0 - tau, where M decreases: ld_bwd = -M.
+ * n_acc, n_rej, status: [2][n_ic] (row 0 forward, row 1 backward) or NULL.  A trajectory whose run does not
+ * end with status 0 gets NaN. */
+int orc_ld_adaptive(int sys, const double *params, long long n_ic, const double *y0, double t0, double tau,
+                    double rtol, double atol, double h0, long long max_steps, double *ld_fwd, double *ld_bwd,
+                    long long *n_acc, long long *n_rej, int *status, int n_threads)
+{
+    int n = orc_dim(sys, params);
+    if (n < 0 || n_ic < 0 || !y0 || !(tau >= 0) || !(rtol > 0) || !(atol > 0)) return ORC_EINVAL;
+    prob_t pb = {sys, params, n, 0, 1};
+    int D = n + 1;
+    if (n_threads < 1) n_threads = 1;
+#pragma omp parallel num_threads(n_threads)
+    {
+        work_t wk;
+        real *Y = malloc(sizeof(real) * (size_t)D);
+        int ok = work_alloc(&wk, D) && Y;
+#pragma omp for schedule(dynamic, 16)
+        for (long long ic = 0; ic < n_ic; ic++) {
+            if (!ok) continue;
+            for (int pass = 0; pass < 2; pass++) {
+                double *out = pass == 0 ? ld_fwd : ld_bwd;
+                if (!out) continue;
+                gather(n_ic, ic, n, 0, y0, NULL, Y);
+                Y[n] = 0;
+                stepper_t st = {1, (real)t0, 0, 0, pass == 0 ? (real)t0 + (real)tau : (real)t0 - (real)tau,
+                                (real)rtol, (real)atol, (real)h0, max_steps};
+                report_t rep = {0, 0, 0, 0, NULL, 0};
+                run_traj(&pb, Y, &st, MODE_NONE, IND_NONE, 1, 0, 1, NULL, 0, NULL, &rep, &wk);
+                int good = rep.status == ST_OK && all_finite(D, Y);
+                out[ic] = good ? (double)(pass == 0 ? Y[n] : -Y[n]) : NAN;
+                if (n_acc) n_acc[(long long)pass * n_ic + ic] = rep.n_acc;
+                if (n_rej) n_rej[(long long)pass * n_ic + ic] = rep.n_rej;
+                if (status) status[(long long)pass * n_ic + ic] = rep.status;
+            }
+        }
+        if (ok) work_free(&wk);
+        free(Y);
+    }
+    return ORC_OK;
+}
+
 /* f(Y) for one augmented state (AoS: y then w_1..w_k) */
 int orc_rhs(int sys, const double *params, int k, const double *Y, double *F)
 {

@@ -55,6 +55,10 @@ def _lib(precision):
         lib.orc_ld_neighbours.restype = C.c_int
         lib.orc_ld_neighbours.argtypes = [C.c_int, _dp, C.c_longlong, _dp, C.c_double, C.c_double, C.c_double,
                                           C.c_longlong, _dp, _dp, _dp, _dp, C.c_int]
+        lib.orc_ld_adaptive.restype = C.c_int
+        lib.orc_ld_adaptive.argtypes = [C.c_int, _dp, C.c_longlong, _dp, C.c_double, C.c_double, C.c_double,
+                                        C.c_double, C.c_double, C.c_longlong, _dp, _dp, C.c_void_p, C.c_void_p,
+                                        C.c_void_p, C.c_int]
         lib.orc_rhs.argtypes = [C.c_int, _dp, C.c_int, _dp, _dp]
         lib.orc_energy.argtypes = [C.c_int, _dp, C.c_longlong, _dp, _dp]
         lib.orc_step.argtypes = [C.c_int, _dp, C.c_int, _dp, C.c_double, _dp, C.c_double, C.c_double, _dp]
@@ -164,6 +168,26 @@ def ld(system, params, y0, t0, h, n_steps, *, forward=True, backward=True, preci
     if rc != 0:
         raise ValueError("orc_ld: invalid arguments")
     return f, b
+
+
+def ld_adaptive(system, params, y0, t0, tau, *, rtol, atol, h0=0.0, max_steps=0, forward=True, backward=True,
+                precision="f64", threads=None):
+    """Arc-length LD over [t0, t0 +- tau] with the adaptive solver on the augmented ODE (y, M), M' = |f|.
+    Returns dict(fwd, bwd [n_ic] or None, n_accepted, n_rejected, status [2, n_ic]: row 0 forward, 1 backward)."""
+    lib = _lib(precision)
+    pr = _params(params)
+    n = dim(system, pr)
+    n_ic = y0.shape[1]
+    _chk(y0, (n, n_ic), "y0")
+    f = np.empty(n_ic) if forward else None
+    b = np.empty(n_ic) if backward else None
+    na, nr = np.zeros((2, n_ic), dtype=np.int64), np.zeros((2, n_ic), dtype=np.int64)
+    st = np.zeros((2, n_ic), dtype=np.int32)
+    rc = lib.orc_ld_adaptive(system, _p(pr), n_ic, _p(y0), t0, tau, rtol, atol, h0, max_steps, _p(f), _p(b),
+                             na.ctypes.data, nr.ctypes.data, st.ctypes.data, threads or default_threads())
+    if rc != 0:
+        raise ValueError("orc_ld_adaptive: invalid arguments")
+    return dict(fwd=f, bwd=b, n_accepted=na, n_rejected=nr, status=st)
 
 
 def ld_neighbours(system, params, y0, sigma, t0, h, n_steps, *, forward=True, backward=True, diffs=True,

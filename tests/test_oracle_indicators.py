@@ -254,6 +254,57 @@ def test_ld_matches_scipy_quadrature(orc):
             assert abs(abs(sol.y[4, -1]) - val) < 1e-10
 
 
+def test_ld_adaptive_closed_form_and_fixed_step_value(orc):
+    """Adaptive LD (augmented ODE, M' = |f|): the isotropic oscillator has |f| = sqrt(2E) constant, so
+    M+ = M- = tau sqrt(2E) whatever the step sequence; on Henon-Heiles the value is the fixed-step
+    quadrature's (a different discretisation of the same integral) and the mirror symmetry holds."""
+    P = np.array([1.0, 1.0, 1.0, 0.0])
+    y = np.random.default_rng(3).uniform(-0.5, 0.5, size=(6, 8))
+    E = 0.5 * (y ** 2).sum(0)
+    r = orc.ld_adaptive(C3, P, y, 0.0, 50.0, rtol=1e-12, atol=1e-12, precision="f64")
+    ref = 50.0 * np.sqrt(2 * E)
+    assert (r["status"] == 0).all()
+    assert np.max(np.abs(r["fwd"] - ref) / ref) < 1e-11 and np.max(np.abs(r["bwd"] - ref) / ref) < 1e-11
+    side = 6
+    y0 = wl.hh_grid(0.125, side, side)
+    f, b = orc.ld(HH, None, y0, 0.0, 0.01, 2000, precision="f80")
+    ra = orc.ld_adaptive(HH, None, y0, 0.0, 20.0, rtol=1e-12, atol=1e-12, precision="f80")
+    assert np.max(np.abs(ra["fwd"] / f - 1)) < 1e-10 and np.max(np.abs(ra["bwd"] / b - 1)) < 1e-10
+    assert np.max(np.abs(ra["bwd"].reshape(side, side) - ra["fwd"].reshape(side, side)[:, ::-1])) < 1e-9
+    assert (ra["n_accepted"] > 100).all() and np.all(y0 == wl.hh_grid(0.125, side, side))
+
+
+def test_ld_adaptive_is_solve_ivp_on_the_augmented_system(orc):
+    """Library pin of the step sequence: solve_ivp(DOP853) on (y, M) with the same tolerances takes the same
+    number of accepted steps and ends at the same M (M takes part in the error norm, D = n + 1); backward in
+    time M decreases and the descriptor is -M."""
+    from scipy.integrate import solve_ivp
+    y0 = np.ascontiguousarray(wl.hh_grid(1.0 / 6.0, 5, 5)[:, [3, 11, 17]])
+    r = orc.ld_adaptive(HH, None, y0, 0.0, 30.0, rtol=1e-9, atol=1e-9, precision="f64", threads=1)
+
+    def fun(t, Y):
+        g = orc.rhs(HH, None, Y[:4])
+        return np.concatenate([g, [np.linalg.norm(g)]])
+    for i in range(3):
+        for row, sgn, val in ((0, 1, r["fwd"][i]), (1, -1, r["bwd"][i])):
+            sol = solve_ivp(fun, (0.0, sgn * 30.0), np.concatenate([y0[:, i], [0.0]]), method="DOP853", rtol=1e-9,
+                            atol=1e-9)
+            assert abs(sgn * sol.y[4, -1] - val) < 1e-11 * val
+            assert abs((len(sol.t) - 1) - r["n_accepted"][row, i]) <= 1
+
+
+def test_ld_adaptive_status_and_arguments(orc):
+    """max_steps exhausted -> status 3 and NaN for that direction; tau = 0 -> M = 0; bad tolerances refused."""
+    y0 = wl.hh_grid(0.125, 3, 3)
+    r = orc.ld_adaptive(HH, None, y0, 0.0, 50.0, rtol=1e-12, atol=1e-12, max_steps=20)
+    assert (r["status"] == 3).all() and np.isnan(r["fwd"]).all() and np.isnan(r["bwd"]).all()
+    assert (r["n_accepted"] + r["n_rejected"] == 20).all()
+    r = orc.ld_adaptive(HH, None, y0, 0.0, 0.0, rtol=1e-9, atol=1e-9)
+    assert (r["fwd"] == 0).all() and (r["bwd"] == 0).all()
+    with pytest.raises(ValueError):
+        orc.ld_adaptive(HH, None, y0, 0.0, 1.0, rtol=0.0, atol=1e-9)
+
+
 # ----------------------------------------------------------------------------- continuation / sampling
 def test_checkpoint_continuation(orc):
     """One call of n steps == two calls of n/2 (split on a renormalisation boundary)."""
