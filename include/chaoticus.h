@@ -142,6 +142,18 @@ int chaoticus_gali(const chs_problem* pb, long long n_ic, double* y, double* w, 
 int chaoticus_ld(const chs_problem* pb, long long n_ic, const double* y0, double t0, double h,
                  long long n_steps, double* ld_fwd, double* ld_bwd, void* stream);
 
+/* The same descriptor with the ADAPTIVE solver (PAPER.md:48 solver 2; PAPER.md:39 the descriptor "calculated
+ * alongside the trajectory's evolution"; R21): the augmented ODE (y, M), M' = |f(y)|_2, M(t0) = 0;
+ * M is one more component of the state and takes part in the error norm (D = n + 1).  st->adaptive must be 1
+ * and st->t_end >= st->t0: tau = t_end - t0; ld_fwd = M over [t0, t0 + tau], ld_bwd over [t0 - tau, t0].
+ *  y0            DEVICE [n][n_ic], NOT modified;  ld_fwd, ld_bwd DEVICE [n_ic], either may be NULL
+ *  rep           optional; its arrays are [2][n_ic] here (row 0 forward, row 1 backward; the row of a direction
+ *                that was not asked for is left untouched); carry / resume are ignored.
+ * A trajectory that does not end with status 0 gets NaN.  Separable systems only (the double pendulum
+ * returns CHS_EUNSUPPORTED). */
+int chaoticus_ld_adaptive(const chs_problem* pb, long long n_ic, const double* y0, const chs_stepper* st,
+                          double* ld_fwd, double* ld_bwd, const chs_report* rep, void* stream);
+
 /* Neighbouring trajectories for the LD-based chaos indicators: for every
  * IC x0 the 1 + 2n members  m = 0: x0;  m = 1 + 2i: x0 + sigma e_i;  m = 2 + 2i: x0 - sigma e_i
  * (e_i: unit vector of phase-space component i in the ordering of y) are generated ON THE DEVICE and
@@ -169,6 +181,8 @@ int chaoticus_lyap(const chs_problem* pb, long long n_ic, double* y, double* w, 
  * They allocate device scratch, copy in, run on an internal stream, copy out and synchronise. */
 int chaoticus_ld_host(const chs_problem* pb, long long n_ic, const double* y0, double t0, double h,
                       long long n_steps, double* ld_fwd, double* ld_bwd);
+int chaoticus_ld_adaptive_host(const chs_problem* pb, long long n_ic, const double* y0, const chs_stepper* st,
+                               double* ld_fwd, double* ld_bwd, const chs_report* rep);
 int chaoticus_ld_neighbours_host(const chs_problem* pb, long long n_ic, const double* y0, double sigma, double t0,
                                  double h, long long n_steps, double* ld_fwd, double* ld_bwd, double* diff_fwd,
                                  double* diff_bwd);

@@ -23,7 +23,8 @@ ST_OK, ST_NONFINITE, ST_UNDERFLOW, ST_MAXSTEPS = 0, 1, 2, 3
 EXPORTS = [
     "chaoticus_version", "chaoticus_last_error", "chaoticus_dim", "chaoticus_n_samples",
     "chaoticus_integrate_fixed", "chaoticus_integrate_adaptive", "chaoticus_sali", "chaoticus_gali",
-    "chaoticus_ld", "chaoticus_ld_neighbours", "chaoticus_ld_neighbours_host", "chaoticus_lyap", "chaoticus_ld_host", "chaoticus_sali_host", "chaoticus_gali_host",
+    "chaoticus_ld", "chaoticus_ld_adaptive", "chaoticus_ld_neighbours", "chaoticus_lyap", "chaoticus_ld_host",
+    "chaoticus_ld_adaptive_host", "chaoticus_ld_neighbours_host", "chaoticus_sali_host", "chaoticus_gali_host",
     "chaoticus_lyap_host", "chaoticus_integrate_host", "chaoticus_kernel_info", "chaoticus_set_option",
 ]
 
@@ -63,6 +64,8 @@ def _load():
     lib.chaoticus_sali.argtypes = [PP, ll, vp, vp, SP, i, i, vp, vp, RP, vp]
     lib.chaoticus_gali.argtypes = [PP, ll, vp, vp, i, SP, i, i, vp, vp, RP, vp]
     lib.chaoticus_ld.argtypes = [PP, ll, vp, dbl, dbl, ll, vp, vp, vp]
+    lib.chaoticus_ld_adaptive.argtypes = [PP, ll, vp, SP, vp, vp, RP, vp]
+    lib.chaoticus_ld_adaptive_host.argtypes = [PP, ll, vp, SP, vp, vp, RP]
     lib.chaoticus_ld_neighbours.argtypes = [PP, ll, vp, dbl, dbl, dbl, ll, vp, vp, vp, vp, vp]
     lib.chaoticus_ld_neighbours_host.argtypes = [PP, ll, vp, dbl, dbl, dbl, ll, vp, vp, vp, vp]
     lib.chaoticus_lyap.argtypes = [PP, ll, vp, vp, i, SP, i, vp, vp, RP, vp]
@@ -238,6 +241,43 @@ def ld(system, params, y0, t0, h, n_steps, *, forward=True, backward=True, out_f
     _check(_lib.chaoticus_ld(C.byref(pb), n_ic, _dev(y0, (n, n_ic), "y0"), t0, h, int(n_steps),
                              _dev(f, (n_ic,), "ld_fwd"), _dev(b, (n_ic,), "ld_bwd"), _stream()))
     return f, b
+
+
+class LdReport(Report):
+    """Report of chaoticus_ld_adaptive: every array is [2, n_ic] (row 0 forward, row 1 backward)."""
+
+    def __init__(self, n_ic, device):
+        self.n_accepted = torch.zeros((2, n_ic), dtype=torch.int64, device=device)
+        self.n_rejected = torch.zeros((2, n_ic), dtype=torch.int64, device=device)
+        self.status = torch.zeros((2, n_ic), dtype=torch.int32, device=device)
+        self.t_final = torch.zeros((2, n_ic), dtype=torch.float64, device=device)
+        self.carry = None
+        self.resume = False
+
+
+def ld_adaptive(system, params, y0, t0, tau, *, rtol, atol, h0=0.0, max_steps=0, forward=True, backward=True,
+                report=None):
+    """Arc-length LD over [t0, t0 +- tau] with the adaptive solver (augmented ODE, M' = |f|).
+    Returns (ld_fwd, ld_bwd), each [n_ic] or None.  y0 is not modified.  report: an LdReport."""
+    pb = _problem(system, params)
+    n = _dim(pb)
+    n_ic = y0.shape[1]
+    st = _stepper(adaptive=True, t0=t0, t_end=t0 + tau, rtol=rtol, atol=atol, h0=h0, max_steps=max_steps)
+    f = torch.empty(n_ic, dtype=torch.float64, device=y0.device) if forward else None
+    b = torch.empty(n_ic, dtype=torch.float64, device=y0.device) if backward else None
+    _check(_lib.chaoticus_ld_adaptive(C.byref(pb), n_ic, _dev(y0, (n, n_ic), "y0"), C.byref(st),
+                                      _dev(f, (n_ic,), "ld_fwd"), _dev(b, (n_ic,), "ld_bwd"), _rep(report), _stream()))
+    return f, b
+
+
+def ld_adaptive_host(system, params, y0, t0, tau, ld_fwd, ld_bwd, *, rtol, atol, h0=0.0, max_steps=0):
+    """HOST buffers (numpy): y0 [n, n_ic]; ld_fwd / ld_bwd [n_ic] or None, filled in place."""
+    pb = _problem(system, params)
+    n = _dim(pb)
+    n_ic = y0.shape[1]
+    st = _stepper(adaptive=True, t0=t0, t_end=t0 + tau, rtol=rtol, atol=atol, h0=h0, max_steps=max_steps)
+    _check(_lib.chaoticus_ld_adaptive_host(C.byref(pb), n_ic, _host(y0, (n, n_ic), "y0"), C.byref(st),
+                                           _host(ld_fwd, (n_ic,), "ld_fwd"), _host(ld_bwd, (n_ic,), "ld_bwd"), None))
 
 
 def ld_neighbours(system, params, y0, sigma, t0, h, n_steps, *, forward=True, backward=True, diffs=True,

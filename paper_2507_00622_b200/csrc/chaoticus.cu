@@ -392,6 +392,67 @@ int chaoticus_ld(const chs_problem* pb, long long n_ic, const double* y0, double
     return ld_common(pb, n_ic, y0, t0, h, n_steps, ld_fwd, ld_bwd, stream, nullptr);
 }
 
+static int ld_adaptive_common(const chs_problem* pb, long long n_ic, const double* y0, const chs_stepper* st,
+                              double* ld_fwd, double* ld_bwd, const chs_report* rep, void* stream,
+                              chs::KernelInfo* info) {
+    int fput_n = 0;
+    const int n = dim_of(pb, &fput_n);
+    if (n < 0) return fail(CHS_EINVAL, "unknown system or bad params");
+    if (n_ic < 0) return fail(CHS_EINVAL, "n_ic < 0");
+    int rc = check_stepper(st, 1);
+    if (rc) return rc;
+    if (!(st->t_end >= st->t0)) return fail(CHS_EINVAL, "ld_adaptive: t_end must be >= t0 (tau = t_end - t0)");
+    if (!info && n_ic > 0 && !y0) return fail(CHS_EINVAL, "y0 is NULL");
+    if (!info && !ld_fwd && !ld_bwd) return CHS_OK;
+    chs::LaunchReq rq;
+    std::memset(&rq, 0, sizeof rq);
+    rq.system = pb->system;
+    rq.what = chs::WHAT_LD;
+    rq.k = 0;
+    rq.adaptive = 1;
+    rq.fput_n = fput_n;
+    rq.params = pb->params;
+    rq.n_params = pb->n_params;
+    rq.tab = make_tab(1.0);
+    rq.stream = (cudaStream_t)stream;
+    rq.info = info;
+    chs::RunArgs& a = rq.args;
+    a.n_ic = n_ic;
+    a.y0 = y0;
+    a.t0 = st->t0;
+    a.t_end = st->t_end;
+    a.rtol = st->rtol;
+    a.atol = st->atol;
+    a.h0 = st->h0;
+    a.max_steps = st->max_steps;
+    a.m = 1;
+    a.n_samples = 1;
+    a.ld_fwd = ld_fwd;
+    a.ld_bwd = ld_bwd;
+    a.dir_first = (info || ld_fwd) ? 0 : 1;
+    a.n_dirs = (info || (ld_fwd && ld_bwd)) ? 2 : 1;
+    if (rep) {
+        a.n_acc = rep->n_accepted;
+        a.n_rej = rep->n_rejected;
+        a.status = rep->status;
+        a.t_final = rep->t_final;
+    }
+    if (n_ic == 0 && !info) return CHS_OK;
+    QueueLease lease;
+    if (!info && g_adaptive_refill.load() != 0) {
+        lease = acquire_queue(rq.stream);
+        a.queue = lease.counter;
+    }
+    const int r = dispatch(rq);
+    release_after_launch(lease, rq.stream);
+    return finish(r, rq);
+}
+
+int chaoticus_ld_adaptive(const chs_problem* pb, long long n_ic, const double* y0, const chs_stepper* st,
+                          double* ld_fwd, double* ld_bwd, const chs_report* rep, void* stream) {
+    return ld_adaptive_common(pb, n_ic, y0, st, ld_fwd, ld_bwd, rep, stream, nullptr);
+}
+
 int chaoticus_ld_neighbours(const chs_problem* pb, long long n_ic, const double* y0, double sigma, double t0,
                             double h, long long n_steps, double* ld_fwd, double* ld_bwd, double* diff_fwd,
                             double* diff_bwd, void* stream) {
@@ -415,7 +476,14 @@ int chaoticus_kernel_info(const chs_problem* pb, int what, int k, int adaptive, 
     if (!info5) return fail(CHS_EINVAL, "info5 is NULL");
     chs::KernelInfo ki{0, 0, 0, 0, 0};
     int rc;
-    if (what == chs::WHAT_LD) {
+    if (what == chs::WHAT_LD && adaptive) {
+        chs_stepper st;
+        std::memset(&st, 0, sizeof st);
+        st.adaptive = 1;
+        st.t_end = 1.0;
+        st.rtol = st.atol = 1e-6;
+        rc = ld_adaptive_common(pb, n_ic, nullptr, &st, nullptr, nullptr, nullptr, nullptr, &ki);
+    } else if (what == chs::WHAT_LD) {
         rc = ld_common(pb, n_ic, nullptr, 0.0, 1.0, 1, nullptr, nullptr, nullptr, &ki);
     } else {
         chs_stepper st;
@@ -570,6 +638,51 @@ int chaoticus_ld_host(const chs_problem* pb, long long n_ic, const double* y0, d
     }
     if (ld_fwd) CK(cudaMemcpyAsync(ld_fwd, df.p, bo, cudaMemcpyDeviceToHost, stream));
     if (ld_bwd) CK(cudaMemcpyAsync(ld_bwd, db.p, bo, cudaMemcpyDeviceToHost, stream));
+    CK(cudaStreamSynchronize(stream));
+    return CHS_OK;
+}
+
+int chaoticus_ld_adaptive_host(const chs_problem* pb, long long n_ic, const double* y0, const chs_stepper* st,
+                               double* ld_fwd, double* ld_bwd, const chs_report* rep) {
+    cudaStream_t stream = nullptr;
+    const int n = dim_of(pb, nullptr);
+    if (n < 0) return fail(CHS_EINVAL, "unknown system or bad params");
+    if (n_ic < 0) return fail(CHS_EINVAL, "n_ic < 0");
+    int rc = check_stepper(st, 1);
+    if (rc) return rc;
+    if (n_ic == 0 || (!ld_fwd && !ld_bwd)) return CHS_OK;
+    if (!y0) return fail(CHS_EINVAL, "y0 is NULL");
+    DevBuf dy, df, db, dacc, drej, dstat, dtf;
+    const size_t by = sizeof(double) * (size_t)n * n_ic, bo = sizeof(double) * (size_t)n_ic;
+    CK(host_stream(&stream));
+    CK(dy.alloc(by, stream));
+    if (ld_fwd) CK(df.alloc(bo, stream));
+    if (ld_bwd) CK(db.alloc(bo, stream));
+    chs_report drep{nullptr, nullptr, nullptr, nullptr, nullptr, 0};
+    if (rep) {  // report arrays are [2][n_ic]
+        if (rep->n_accepted) { CK(dacc.alloc(2 * sizeof(long long) * n_ic, stream)); drep.n_accepted = (long long*)dacc.p; }
+        if (rep->n_rejected) { CK(drej.alloc(2 * sizeof(long long) * n_ic, stream)); drep.n_rejected = (long long*)drej.p; }
+        if (rep->status) { CK(dstat.alloc(2 * sizeof(int) * n_ic, stream)); drep.status = (int*)dstat.p; }
+        if (rep->t_final) { CK(dtf.alloc(2 * sizeof(double) * n_ic, stream)); drep.t_final = (double*)dtf.p; }
+        if (dacc.p) CK(cudaMemsetAsync(dacc.p, 0, dacc.bytes, stream));
+        if (drej.p) CK(cudaMemsetAsync(drej.p, 0, drej.bytes, stream));
+        if (dstat.p) CK(cudaMemsetAsync(dstat.p, 0, dstat.bytes, stream));
+        if (dtf.p) CK(cudaMemsetAsync(dtf.p, 0, dtf.bytes, stream));
+    }
+    CK(cudaMemcpyAsync(dy.p, y0, by, cudaMemcpyHostToDevice, stream));
+    rc = chaoticus_ld_adaptive(pb, n_ic, (const double*)dy.p, st, (double*)df.p, (double*)db.p, &drep, stream);
+    if (rc) {
+        cudaStreamSynchronize(stream);
+        return rc;
+    }
+    if (ld_fwd) CK(cudaMemcpyAsync(ld_fwd, df.p, bo, cudaMemcpyDeviceToHost, stream));
+    if (ld_bwd) CK(cudaMemcpyAsync(ld_bwd, db.p, bo, cudaMemcpyDeviceToHost, stream));
+    if (rep) {
+        if (rep->n_accepted) CK(cudaMemcpyAsync(rep->n_accepted, dacc.p, dacc.bytes, cudaMemcpyDeviceToHost, stream));
+        if (rep->n_rejected) CK(cudaMemcpyAsync(rep->n_rejected, drej.p, drej.bytes, cudaMemcpyDeviceToHost, stream));
+        if (rep->status) CK(cudaMemcpyAsync(rep->status, dstat.p, dstat.bytes, cudaMemcpyDeviceToHost, stream));
+        if (rep->t_final) CK(cudaMemcpyAsync(rep->t_final, dtf.p, dtf.bytes, cudaMemcpyDeviceToHost, stream));
+    }
     CK(cudaStreamSynchronize(stream));
     return CHS_OK;
 }

@@ -59,6 +59,8 @@ struct RunArgs {
     // 1 + 2n = centre and x0 +- sigma e_i), outputs are [member][ic]
     int n_members;
     double sigma;
+    // adaptive LD (run_kernel<..., LD = true>): which directions the tasks cover (0 forward, 1 backward)
+    int dir_first, n_dirs;
     // adaptive runs: work queue for lane refill (device counter, zeroed before the launch), or null
     unsigned long long* queue;
 };
@@ -525,14 +527,54 @@ struct LdHook {
     }
 };
 
+// The same norms inside an ADAPTIVE attempt (scaled forces G = h^2 F, raw table): after stage i with b_i != 0
+// keep |k_i|_2 = |(P_i, F_i)|_2, P_i = p + (1/h) sum_j a_ij G_j, F_i = G_i / h^2; the attempt then forms
+// M+ = M + |h| sum b_i |k_i| and the embedded errors of M from the same eight numbers (b, E5 and E3 share
+// their support).
+template <class C>
+struct LdNormHook {
+    const Tab& tab;
+    const C& s;
+    double hinv, hinv2;
+    double (&nrm)[12];
+    template <int i>
+    __device__ __forceinline__ void operator()(Int<i>, const double (&F)[12][C::NI]) const {
+        if constexpr (coef::B[i] != 0.0) {
+            double n2 = 0.0;
+#pragma unroll
+            for (int c = 0; c < C::NI; c++) {
+                double P = s.p[c];
+                if constexpr (i > 0) {
+                    double sum = 0.0;
+                    bool first = true;
+                    static_for<0, i>([&](auto jc) {
+                        constexpr int j = decltype(jc)::value;
+                        if constexpr (coef::A[i][j] != 0.0) {
+                            sum = first ? tab.ap[i][j] * F[j][c] : fma(tab.ap[i][j], F[j][c], sum);
+                            first = false;
+                        }
+                    });
+                    P = fma(hinv, sum, P);
+                }
+                const double f = F[i][c] * hinv2;
+                n2 = fma(P, P, fma(f, f, n2));
+            }
+            nrm[i] = fast_sqrt(tile_sum<C::L>(n2));
+        }
+    }
+};
+
 // ---- the run kernel: fixed or adaptive, with renormalisation / indicator ----------------------
 // S = the per-lane state class of a layout (Col<Sys,K,L> here, Chain<NP,K> in chain_kernels.cuh)
 // PAIR: evaluate the stages two at a time (dop8_core.cuh dop8_stages); off only where the extra live
 // stage vector does not fit the register file.
-template <class C, int MODE, int IND, bool ADAPT, int TPB, int MINB, bool PAIR = true>
+// LD (adaptive only, K = 0): the arc-length Lagrangian descriptor rides along as one more component of the state
+// (R21): tasks are (direction, IC) pairs, nothing is written back but M and the report.
+template <class C, int MODE, int IND, bool ADAPT, int TPB, int MINB, bool PAIR = true, bool LD = false>
 __global__ void __launch_bounds__(TPB, MINB)
 run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const RunArgs a) {
     constexpr int NI = C::NI, L = C::L, K = C::K;
+    static_assert(!LD || (ADAPT && K == 0 && MODE == MODE_NONE && IND == IND_NONE), "LD rides on the plain adaptive run");
     const long long gt = (long long)blockIdx.x * TPB + threadIdx.x;
     const long long traj = gt / L;
     const bool want_log = (a.logacc != nullptr) || (a.lambda != nullptr);
@@ -666,6 +708,9 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
         bool rejected = false, need = true, fin = false, done = false, first_fetch = true;
         bool more = false;  // t has not reached t_end yet
         int cd = a.m;
+        const long long n_items = LD ? a.n_ic * a.n_dirs : a.n_ic;  // LD: tasks ordered [direction][ic]
+        double M = 0.0;                                              // LD: the descriptor of this task
+        long long out_slot = 0;                                      // LD: row (0 fwd, 1 bwd) * n_ic + ic
         // One vote per iteration: the block below (write out the trajectories that ended in the previous
         // attempt, fetch new ones, leave when nothing is left) is entered only when some tile asks for it.
         while (true) {
@@ -677,22 +722,34 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
                     if constexpr (IND != IND_NONE) ind = s.template indicator<IND>();
                     if (fin) {
                         const int st_out = (bad && status == ST_OK) ? (int)ST_NONFINITE : status;
-                        s.store(a.y, a.w, a.n_ic, ic, bad);
-                        if constexpr (K > 0) s.store_logs(a, ic, bad, t - a.t0);
-                        if (s.lt == 0) {
-                            if constexpr (IND != IND_NONE) {
-                                if (a.series) a.series[ic] = bad ? nan("") : ind;  // adaptive: n_samples = 1
+                        if constexpr (LD) {
+                            bad = bad || !isfinite(M);
+                            if (s.lt == 0) {
+                                double* out = out_slot < a.n_ic ? a.ld_fwd : a.ld_bwd;
+                                out[ic] = bad ? nan("") : M;
+                                if (a.n_acc) a.n_acc[out_slot] = n_acc;
+                                if (a.n_rej) a.n_rej[out_slot] = n_rej;
+                                if (a.status) a.status[out_slot] = (bad && st_out == ST_OK) ? (int)ST_NONFINITE : st_out;
+                                if (a.t_final) a.t_final[out_slot] = t;
                             }
-                            if (a.n_acc) a.n_acc[ic] = n_acc;
-                            if (a.n_rej) a.n_rej[ic] = n_rej;
-                            if (a.status) a.status[ic] = st_out;
-                            if (a.t_final) a.t_final[ic] = t;
+                        } else {
+                            s.store(a.y, a.w, a.n_ic, ic, bad);
+                            if constexpr (K > 0) s.store_logs(a, ic, bad, t - a.t0);
+                            if (s.lt == 0) {
+                                if constexpr (IND != IND_NONE) {
+                                    if (a.series) a.series[ic] = bad ? nan("") : ind;  // adaptive: n_samples = 1
+                                }
+                                if (a.n_acc) a.n_acc[ic] = n_acc;
+                                if (a.n_rej) a.n_rej[ic] = n_rej;
+                                if (a.status) a.status[ic] = st_out;
+                                if (a.t_final) a.t_final[ic] = t;
+                            }
                         }
                         need = true;
                         fin = false;
                     }
                 }
-                long long nxt = a.n_ic;  // "nothing left"
+                long long nxt = n_items;  // "nothing left"
                 if (a.queue != nullptr) {
                     if (need && s.lt == 0) nxt = (long long)atomicAdd(a.queue, 1ULL);
                     nxt = tile_bcast_ll<L>(nxt, 0);
@@ -700,11 +757,19 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
                     nxt = traj;
                 }
                 first_fetch = false;
-                const bool got = need && nxt < a.n_ic;
+                const bool got = need && nxt < n_items;
                 if (need && !got) done = true;
                 if (got) {
-                    ic = nxt;
-                    s.load(a.y, a.w, a.n_ic, ic, 1.0);
+                    if constexpr (LD) {  // backward = forward of the momentum-reversed IC (ld_kernel)
+                        const int dsel = a.dir_first + (int)(nxt / a.n_ic);
+                        ic = nxt % a.n_ic;
+                        out_slot = (long long)dsel * a.n_ic + ic;
+                        s.load(a.y0, nullptr, a.n_ic, ic, dsel == 0 ? 1.0 : -1.0);
+                        M = 0.0;
+                    } else {
+                        ic = nxt;
+                        s.load(a.y, a.w, a.n_ic, ic, 1.0);
+                    }
                     s.reset_logs();
                     t = a.t0;
                     more = interval > 0.0;
@@ -748,8 +813,15 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
 #pragma unroll
             for (int c = 0; c < NI; c++) u[c] = h * s.p[c];
             double F[12][NI];
-            dop8_stages<NI, PAIR>(tab, s.q, u, F, force_h2, nohook);
-            const double hinv = fwd ? fast_rcp(h_try) : -fast_rcp(h_try);  // (h = 0: inf; nothing is committed)
+            double hinv, nrm[LD ? 12 : 1];
+            if constexpr (LD) {
+                hinv = fwd ? fast_rcp(h_try) : -fast_rcp(h_try);
+                const LdNormHook<C> ldhook{tab, s, hinv, hinv * hinv, nrm};
+                dop8_stages<NI, PAIR>(tab, s.q, u, F, force_h2, ldhook);
+            } else {
+                dop8_stages<NI, PAIR>(tab, s.q, u, F, force_h2, nohook);
+                hinv = fwd ? fast_rcp(h_try) : -fast_rcp(h_try);  // (h = 0: inf; nothing is committed)
+            }
             double qn[NI], pn[NI];
             dop8_solution<NI, C::NCOMP, false>(tab, hinv, s.q, s.p, u, F, qn, pn, qc, pc, qcn, pcn);
             double S5, S3;
@@ -762,7 +834,25 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
             }
             // err = |h| S5 / sqrt(D (S5 + 0.01 S3)) against 1, and the step-size factor 0.9 err^(-1/8), without
             // forming err (dop8_core.cuh "step-size controller"): accept <=> num^2 < den
-            const StepDecision dec = step_decision(h_try, S5, S3, s.dcount(), rejected);
+            double Mn = 0.0;
+            if constexpr (LD) {  // M+ and its embedded errors (divided by h, like the sums above)
+                double sb = 0.0, s5 = 0.0, s3 = 0.0;
+                static_for<0, 12>([&](auto ic2) {
+                    constexpr int i = decltype(ic2)::value;
+                    if constexpr (coef::B[i] != 0.0) {
+                        sb = fma(tab.bl[i], nrm[i], sb);
+                        s5 = fma(tab.e5p[i], nrm[i], s5);
+                        s3 = fma(tab.e3p[i], nrm[i], s3);
+                    }
+                });
+                Mn = fma(h_try, sb, M);
+                const double isc = fast_rcp(fma(a.rtol, fmax(fabs(M), fabs(Mn)), a.atol));
+                s5 *= isc;
+                s3 *= isc;
+                S5 = fma(s5, s5, S5);
+                S3 = fma(s3, s3, S3);
+            }
+            const StepDecision dec = step_decision(h_try, S5, S3, s.dcount() + (LD ? 1.0 : 0.0), rejected);
             const bool acc = active && dec.acc, rej = active && dec.rej;
             if (active && !acc && !rej) status = ST_NONFINITE;  // NaN: inf or NaN in y+ (fast_rcp(inf) is NaN)
             if (acc || rej) h_abs = h_try * dec.factor;
@@ -770,6 +860,7 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
             n_acc += acc ? 1 : 0;
             n_rej += rej ? 1 : 0;
             t = acc ? t_new : t;
+            if constexpr (LD) M = acc ? Mn : M;
             more = fwd ? (t < a.t_end) : (t > a.t_end);
 #pragma unroll
             for (int c = 0; c < NI; c++) {

@@ -46,6 +46,15 @@ int run_chain_ld_t(const LaunchReq& rq) {
     return (int)cudaGetLastError();
 }
 
+template <int LT, int PPL, bool PAD, int TPB, int MINB>
+int run_chain_ld_adapt_t(const LaunchReq& rq) {
+    static_assert(LT <= 32 || LT == TPB, "a wide tile is the whole thread block");
+    FputParams prm;
+    if (!fput_params(rq, prm)) return (int)cudaErrorInvalidValue;
+    if (rq.fput_n > LT * PPL || (!PAD && rq.fput_n != LT * PPL)) return (int)cudaErrorInvalidValue;
+    return launch_ld_adapt<Chain<LT, PPL, 0, PAD>, FputParams, TPB, MINB>(rq, prm);
+}
+
 // Lyapunov spectrum with NB K vectors on NB column blocks (chain_kernels.cuh): fixed step, Gram-Schmidt
 template <int LT, int PPL, bool PAD, int KB, int NB, int TPB, int MINB, bool COLD = false>
 int run_chain_blocks(const LaunchReq& rq) {
@@ -73,6 +82,7 @@ int fput_basic_set(const LaunchReq& rq) {
     if (w == WHAT_INTEGRATE && k == 0 && !ad) return run_chain_t<H, 2, PAD, 0, MODE_NONE, IND_NONE, false, 128, 4>(rq);
     if (w == WHAT_INTEGRATE && k == 0 && ad) return run_chain_t<H, 2, PAD, 0, MODE_NONE, IND_NONE, true, 128, 2>(rq);
     if (w == WHAT_LD && k == 0 && !ad) return run_chain_ld_t<H, 2, PAD, 128, 4>(rq);
+    if (w == WHAT_LD && k == 0 && ad) return run_chain_ld_adapt_t<H, 2, PAD, 128, 2>(rq);
     if (w == WHAT_SALI && k == 2 && !ad) return run_chain_t<H, 2, PAD, 2, MODE_NORM, IND_SALI, false, 128, 2>(rq);
     if (w == WHAT_GALI && k == 4 && !ad) return run_chain_t<H, 2, PAD, 4, MODE_NORM, IND_GALI, false, 128, 2, true>(rq);
     if constexpr (NS <= 32) {  // one particle per lane: these need more registers per pair
@@ -89,6 +99,7 @@ int fput_wide_set(const LaunchReq& rq) {
     if (w == WHAT_INTEGRATE && k == 0 && !ad) return run_chain_t<TPB, 1, true, 0, MODE_NONE, IND_NONE, false, TPB, MINB>(rq);
     if (w == WHAT_INTEGRATE && k == 0 && ad) return run_chain_t<TPB, 1, true, 0, MODE_NONE, IND_NONE, true, TPB, MINB>(rq);
     if (w == WHAT_LD && k == 0 && !ad) return run_chain_ld_t<TPB, 1, true, TPB, MINB>(rq);
+    if (w == WHAT_LD && k == 0 && ad) return run_chain_ld_adapt_t<TPB, 1, true, TPB, MINB>(rq);
     if (w == WHAT_SALI && k == 2 && !ad) return run_chain_t<TPB, 1, true, 2, MODE_NORM, IND_SALI, false, TPB, MINB>(rq);
     if (w == WHAT_GALI && k == 4 && !ad) return run_chain_t<TPB, 1, true, 4, MODE_NORM, IND_GALI, false, TPB, MINB>(rq);
     if (w == WHAT_GALI && k == 4 && ad) return run_chain_t<TPB, 1, true, 4, MODE_NORM, IND_GALI, true, TPB, 1>(rq);

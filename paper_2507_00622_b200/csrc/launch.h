@@ -116,6 +116,25 @@ inline int run_ld(const LaunchReq& rq) {
     return (int)cudaGetLastError();
 }
 
+// adaptive Lagrangian descriptor (run_kernel<..., LD = true>): tasks = (direction, IC) pairs
+template <class C, class Params, int TPB, int MINB>
+inline int launch_ld_adapt(const LaunchReq& rq, const Params& prm) {
+    auto kern = run_kernel<C, MODE_NONE, IND_NONE, true, TPB, MINB, true, true>;
+    const long long n_threads = rq.args.n_ic * rq.args.n_dirs * C::L;
+    int r = finish_launch(rq, kern, TPB, C::L, n_threads);
+    if (r != -2) return r;
+    const long long blocks = run_grid(rq, kern, TPB, n_threads);
+    if (blocks == 0) return 0;
+    kern<<<(unsigned)blocks, TPB, 0, rq.stream>>>(rq.tab, prm, rq.args);
+    return (int)cudaGetLastError();
+}
+template <class Sys, int TPB, int MINB>
+inline int run_col_ld_adapt(const LaunchReq& rq) {
+    typename Sys::Params prm;
+    if (!Sys::make_params(rq.params, rq.n_params, prm)) return (int)cudaErrorInvalidValue;
+    return launch_ld_adapt<Col<Sys, 0, 1>, typename Sys::Params, TPB, MINB>(rq, prm);
+}
+
 #define CHS_MATCH(SYSID, WHAT, KK, AD) (rq.system == (SYSID) && rq.what == (WHAT) && rq.k == (KK) && rq.adaptive == (AD))
 
 }  // namespace chs

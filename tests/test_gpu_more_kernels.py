@@ -570,3 +570,79 @@ def test_fput_spectrum_column_blocks(chs, orc, N, k):
     a_y, a_w = dev(y0), dev(w0)
     chs.lyap(FPUT, prm, a_y, a_w, renorm_every=10, h=0.05, n_steps=1203)
     assert torch.equal(a_y, b_y)
+
+
+# ------------------------------------------------------------------ adaptive Lagrangian descriptor (R21)
+@pytest.mark.parametrize("case", ["hh", "coupled3", "fput8", "fput12_padded", "fput100_wide"])
+def test_ld_adaptive(chs, orc, case):
+    """chaoticus_ld_adaptive (augmented ODE (y, M), M' = |f|, M in the error norm) against the oracle's
+    orc_ld_adaptive: two solutions to the same tolerance (R16), so values agree to 1e-8 relative and the
+    accepted counts to 0.5 %; ragged ensemble sizes; both directions and each alone."""
+    if case == "hh":
+        sysid, prm, y0, tau = HH, None, W.hh_grid(1.0 / 6.0, 23, 19), 60.0
+    elif case == "coupled3":
+        cfg = W.config("C4", n_ic=333)
+        sysid, prm, y0, tau = C3, cfg["params"], cfg["y"], 40.0
+    else:
+        N = {"fput8": 8, "fput12_padded": 12, "fput100_wide": 100}[case]
+        n_ic = 37 if N == 100 else 301
+        sysid, prm, y0, tau = FPUT, W.fput_params(N, 1.0, 0.25, 1.0), W.fput_ics(n_ic, N, 7, 1.0), 15.0
+    n_ic = y0.shape[1]
+    tol = 1e-11
+    ro = orc.ld_adaptive(sysid, prm, y0, 0.5, tau, rtol=tol, atol=tol, precision="f80")
+    rep = chs.LdReport(n_ic, "cuda")
+    yg = dev(y0)
+    f, b = chs.ld_adaptive(sysid, prm, yg, 0.5, tau, rtol=tol, atol=tol, report=rep)
+    f, b = f.cpu().numpy(), b.cpu().numpy()
+    assert (rep.status.cpu().numpy() == 0).all() and (ro["status"] == 0).all()
+    assert np.abs(f / ro["fwd"] - 1).max() <= 1e-8 and np.abs(b / ro["bwd"] - 1).max() <= 1e-8
+    na = rep.n_accepted.cpu().numpy()
+    assert abs(na.sum() / ro["n_accepted"].sum() - 1) <= 5e-3
+    assert (rep.t_final.cpu().numpy() == 0.5 + tau).all()     # backward = forward pass of the reversed momenta
+    assert np.array_equal(yg.cpu().numpy(), y0)                # y0 untouched
+    # one direction alone gives the same bits, and leaves the other row of the report untouched
+    rep1 = chs.LdReport(n_ic, "cuda")
+    f1, none = chs.ld_adaptive(sysid, prm, yg, 0.5, tau, rtol=tol, atol=tol, backward=False, report=rep1)
+    assert none is None and np.array_equal(f1.cpu().numpy(), f)
+    assert (rep1.n_accepted[1] == 0).all() and torch_equal(rep1.n_accepted[0], rep.n_accepted[0])
+    none, b1 = chs.ld_adaptive(sysid, prm, yg, 0.5, tau, rtol=tol, atol=tol, forward=False)
+    assert none is None and np.array_equal(b1.cpu().numpy(), b)
+
+
+def torch_equal(a, b):
+    import torch
+    return torch.equal(a, b)
+
+
+def test_ld_adaptive_closed_form_status_and_host(chs):
+    """Isotropic oscillator: M = tau sqrt(2E) whatever the steps; max_steps exhausted -> status 3 and NaN;
+    tau = 0 -> 0; refill on/off bit-identical; host-buffer form equals the device form; error paths."""
+    P = np.array([1.0, 1.0, 1.0, 0.0])
+    y0 = np.random.default_rng(3).uniform(-0.5, 0.5, size=(6, 517))
+    ref = 50.0 * np.sqrt((y0 ** 2).sum(0))
+    yg = dev(y0)
+    f, b = chs.ld_adaptive(C3, P, yg, 0.0, 50.0, rtol=1e-12, atol=1e-12)
+    assert np.abs(f.cpu().numpy() / ref - 1).max() <= 1e-11 and np.abs(b.cpu().numpy() / ref - 1).max() <= 1e-11
+    rep = chs.LdReport(517, "cuda")
+    f2, b2 = chs.ld_adaptive(C3, P, yg, 0.0, 50.0, rtol=1e-12, atol=1e-12, max_steps=25, report=rep)
+    assert (rep.status.cpu().numpy() == 3).all() and np.isnan(f2.cpu().numpy()).all() and np.isnan(b2.cpu().numpy()).all()
+    assert ((rep.n_accepted + rep.n_rejected).cpu().numpy() == 25).all()
+    f0, b0 = chs.ld_adaptive(C3, P, yg, 1.0, 0.0, rtol=1e-9, atol=1e-9)
+    assert (f0 == 0).all().item() and (b0 == 0).all().item()
+    try:
+        chs.set_option("adaptive_refill", 0)
+        f3, b3 = chs.ld_adaptive(C3, P, yg, 0.0, 50.0, rtol=1e-12, atol=1e-12)
+    finally:
+        chs.set_option("adaptive_refill", 1)
+    assert torch_equal(f3, f) and torch_equal(b3, b)
+    fh, bh = np.empty(517), np.empty(517)
+    chs.ld_adaptive_host(C3, P, y0, 0.0, 50.0, fh, bh, rtol=1e-12, atol=1e-12)
+    assert np.array_equal(fh, f.cpu().numpy()) and np.array_equal(bh, b.cpu().numpy())
+    with pytest.raises(chs.ChaoticusError):
+        chs.ld_adaptive(C3, P, yg, 0.0, -1.0, rtol=1e-9, atol=1e-9)          # tau < 0
+    with pytest.raises(chs.ChaoticusError):
+        chs.ld_adaptive(C3, P, yg, 0.0, 1.0, rtol=0.0, atol=1e-9)
+    with pytest.raises(chs.ChaoticusError):                                    # not separable: no kernel
+        chs.ld_adaptive(W.SYS_DOUBLE_PENDULUM, (1.0, 1.0), dev(W.double_pendulum_ics(8, seed=1)), 0.0, 1.0,
+                        rtol=1e-9, atol=1e-9)
+    assert chs.kernel_info(HH, None, chs.WHAT_LD, adaptive=True, n_ic=1000)["spill_bytes"] == 0
