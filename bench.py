@@ -38,7 +38,7 @@ METRIC = "trajectory RK-steps/sec (FP64, incl. variational eqs)"
 UNIT = "RK-steps/s"
 # algorithmic FP64 flop per RK-step of the formulation that runs
 FLOP_PER_STEP = {"C1": 1216.0, "C2": 640.0, "C1sat": 1216.0, "C3": 1746.0, "C4": 4213.0, "C5": 8492.0, "F3": None,
-                 "F1": None, "LDN": 640.0}
+                 "F1": None, "LDN": 640.0, "LDA": None}
 WORKLOAD_LABEL = {
     "C1": "C1: Henon-Heiles E=1/8, 32x32 grid (1024 ICs), fixed DOP8 h=0.01, 1e4 steps, SALI renormalised every step",
     "C2": "C2: Henon-Heiles Lagrangian descriptor (arc length), E=1/8, 1024x1024 grid per GPU, fixed DOP8 h=0.01, 5000 steps forward + 5000 backward",
@@ -48,6 +48,7 @@ WORKLOAD_LABEL = {
     "C5": "C5: FPUT-beta N=8, 65536 ICs, GALI_4 (renormalised every 10 steps), h=0.05, 2e4 steps",
     "F1": "F1 (shape of PAPER.md Fig. 1): dimensionless double pendulum (sigma = alpha = 1), random ICs, t = 1000, fixed h = 0.01 or adaptive rtol = atol = 1e-9",
     "F3": "F3 (shape of PAPER.md Fig. 3): FPUT-beta chain, random ICs, GALI_4, adaptive DOP8(5) rtol=atol=1e-8, t=1000",
+    "LDA": "LDA: the C2 grid with the ADAPTIVE solver (chaoticus_ld_adaptive: augmented ODE (y, M), rtol=atol=1e-10), tau = h * --n-steps forward + backward (RK-step = attempted step)",
     "LDN": "LDN: LD of every IC of the C2 grid and of its 2n axis neighbours x0 +- sigma e_i, generated on the device (PAPER.md:57-58), fixed DOP8 h=0.01, --n-steps steps forward + backward",
 }
 PER_CONFIG = ["C1", "C1sat", "C2", "C3", "C4", "C5"]
@@ -183,7 +184,7 @@ def kernel_traffic(workload):
 
 def workload_inputs(args, rank, world):
     from paper_2507_00622_b200 import workloads as W
-    if args.workload in ("C2", "LDN"):
+    if args.workload in ("C2", "LDN", "LDA"):
         side = args.side
         y0 = W.hh_grid(0.125, side * world, side, i_range=(rank * side, (rank + 1) * side))
         return dict(y0=y0, h=0.01, n_steps=args.n_steps, rk_steps=2.0 * y0.shape[1] * args.n_steps)
@@ -335,7 +336,7 @@ def make_workload(chs, torch, args, rank, world, name=None):
         return dict(wl=wl, n_ic=n_ic, h2d=y0_host.numel() * 8, d2h=y0_host.numel() * 8,
                     kinfo=chs.kernel_info(DPS, prm, chs.WHAT_INTEGRATE, adaptive=args.f1_adaptive, n_ic=n_ic),
                     step_dev=call, step_e2e=step_e2e, prepare=lambda: yb.copy_(y0))
-    if name in ("C2", "LDN"):
+    if name in ("C2", "LDN", "LDA"):
         wl = workload_inputs(args, rank, world)
         y0_host = torch.from_numpy(wl["y0"]).pin_memory()
         y0 = y0_host.cuda()
@@ -349,6 +350,16 @@ def make_workload(chs, torch, args, rank, world, name=None):
                     kinfo=chs.kernel_info(HH, None, chs.WHAT_LD, n_ic=n_ic),
                     step_dev=lambda: chs.ld(HH, None, y0, 0.0, wl["h"], wl["n_steps"], out_fwd=f, out_bwd=b),
                     step_e2e=lambda: chs.ld_host(HH, None, y0_host, 0.0, wl["h"], wl["n_steps"], f_host, b_host))
+    if name == "LDA":
+        tau = wl["h"] * wl["n_steps"]
+        rep = chs.LdReport(n_ic, "cuda")
+        f_host = torch.empty(n_ic, dtype=torch.float64).pin_memory()
+        b_host = torch.empty(n_ic, dtype=torch.float64).pin_memory()
+        wl = dict(wl, rk_steps=None, report=rep)
+        return dict(wl=wl, n_ic=n_ic, h2d=y0_host.numel() * 8, d2h=2 * n_ic * 8,
+                    kinfo=chs.kernel_info(HH, None, chs.WHAT_LD, adaptive=True, n_ic=n_ic),
+                    step_dev=lambda: chs.ld_adaptive(HH, None, y0, 0.0, tau, rtol=1e-10, atol=1e-10, report=rep),
+                    step_e2e=lambda: chs.ld_adaptive_host(HH, None, y0_host, 0.0, tau, f_host, b_host, rtol=1e-10, atol=1e-10))
     if name == "LDN":
         nn = 1 + 2 * 4
         f = torch.empty((nn, n_ic), dtype=torch.float64, device="cuda")

@@ -646,3 +646,42 @@ def test_ld_adaptive_closed_form_status_and_host(chs):
         chs.ld_adaptive(W.SYS_DOUBLE_PENDULUM, (1.0, 1.0), dev(W.double_pendulum_ics(8, seed=1)), 0.0, 1.0,
                         rtol=1e-9, atol=1e-9)
     assert chs.kernel_info(HH, None, chs.WHAT_LD, adaptive=True, n_ic=1000)["spill_bytes"] == 0
+
+
+def test_adaptive_status_words_match_the_oracle(chs, orc):
+    """The controller's corner cases against the oracle on identical inputs (the kernels build 10 ulp(t) from
+    integer instructions and take the accept decision without forming err, the oracle uses nextafter and pow):
+    step-size underflow at t0 = 1e17 (10 ulp = 160: one rejected attempt, nothing accepted, t unchanged), at
+    a negative t0 and backwards in time; max_steps hit at exactly the same attempt; blow-up time of an escaping
+    orbit within the solver's resolution."""
+    y0 = np.ascontiguousarray(W.hh_grid(0.125, 4, 4)[:, 5:8])
+    for t0, t_end in ((1e17, 1e17 + 1e6), (-1e17, -1e17 + 1e6), (1e17, 1e17 - 1e6), (-4.0e16, -4.0e16 - 1e6)):
+        yo = y0.copy()
+        ro = orc.integrate_adaptive(HH, None, yo, t0, t_end, 1e-9, 1e-9, h0=160.0, precision="f64")
+        yg, rep = dev(y0), chs.Report(3, "cuda")
+        chs.integrate_adaptive(HH, None, yg, t0, t_end, 1e-9, 1e-9, h0=160.0, report=rep)
+        assert (ro["status"] == chs.ST_UNDERFLOW).all()
+        assert (rep.status.cpu().numpy() == ro["status"]).all()
+        assert (rep.n_accepted.cpu().numpy() == ro["n_accepted"]).all() and (rep.n_rejected.cpu().numpy() == ro["n_rejected"]).all()
+        assert (rep.t_final.cpu().numpy() == t0).all() and np.isnan(yg.cpu().numpy()).all()
+    # max_steps: same count of attempts on both sides, same status
+    y0 = W.hh_grid(0.125, 6, 6)
+    yo = y0.copy()
+    ro = orc.integrate_adaptive(HH, None, yo, 0.0, 100.0, 1e-10, 1e-10, max_steps=57, precision="f64")
+    yg, rep = dev(y0), chs.Report(36, "cuda")
+    chs.integrate_adaptive(HH, None, yg, 0.0, 100.0, 1e-10, 1e-10, max_steps=57, report=rep)
+    assert (ro["status"] == chs.ST_MAXSTEPS).all() and (rep.status.cpu().numpy() == chs.ST_MAXSTEPS).all()
+    assert ((rep.n_accepted + rep.n_rejected).cpu().numpy() == 57).all()
+    assert np.abs(rep.t_final.cpu().numpy() - ro["t_final"]).max() <= 1e-6 * ro["t_final"].max()
+    # escaping orbit: flagged at the same time
+    y0 = W.hh_grid(0.125, 3, 3).copy()
+    y0[:, 4] = [0.0, 3.0, 0.0, 5.0]
+    yo = y0.copy()
+    ro = orc.integrate_adaptive(HH, None, yo, 0.0, 50.0, 1e-10, 1e-10, max_steps=200000, precision="f64")
+    yg, rep = dev(y0), chs.Report(9, "cuda")
+    chs.integrate_adaptive(HH, None, yg, 0.0, 50.0, 1e-10, 1e-10, max_steps=200000, report=rep)
+    st = rep.status.cpu().numpy()
+    assert st[4] in (chs.ST_NONFINITE, chs.ST_UNDERFLOW) and ro["status"][4] in (chs.ST_NONFINITE, chs.ST_UNDERFLOW)
+    assert abs(rep.t_final.cpu().numpy()[4] - ro["t_final"][4]) < 1e-3
+    ok = np.delete(np.arange(9), 4)
+    assert (st[ok] == 0).all() and rel_state(yg.cpu().numpy()[:, ok], yo[:, ok]).max() <= 1e-8
