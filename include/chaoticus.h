@@ -123,7 +123,9 @@ int chaoticus_integrate_adaptive(const chs_problem* pb, long long n_ic, double* 
  *  w        DEVICE [2][n][n_ic] in/out; normalised once on entry
  *  sali     DEVICE [n_samples][n_ic]; row s < n_samples-1 = value after the
  *           (s+1)*sample_every-th renormalisation, last row = value at the end.
- *           sample_every must be 0 for adaptive runs (n_samples = 1).
+ *           sample_every must be 0 for adaptive runs (n_samples = 1): their accepted times differ per
+ *           trajectory.  A time series of an adaptive run is taken by continuation -- consecutive calls
+ *           t_j -> t_{j+1} with rep->resume = 1 (each lands on its checkpoint exactly).
  *  lognorm  DEVICE [2][n_ic] or NULL; the run ADDS sum ln|w_v| of its renormalisations. */
 int chaoticus_sali(const chs_problem* pb, long long n_ic, double* y, double* w, const chs_stepper* st,
                    int renorm_every, int sample_every, double* sali, double* lognorm,

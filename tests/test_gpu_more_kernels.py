@@ -685,3 +685,36 @@ def test_adaptive_status_words_match_the_oracle(chs, orc):
     assert abs(rep.t_final.cpu().numpy()[4] - ro["t_final"][4]) < 1e-3
     ok = np.delete(np.arange(9), 4)
     assert (st[ok] == 0).all() and rel_state(yg.cpu().numpy()[:, ok], yo[:, ok]).max() <= 1e-8
+
+
+def test_adaptive_indicator_time_series_by_continuation(chs, orc):
+    """An indicator time series of an ADAPTIVE run (sample_every must be 0 there: accepted times differ per
+    trajectory) is taken by continuation: consecutive calls t_j -> t_{j+1} with resume = 1 (no entry
+    normalisation; the last step of each call lands on the checkpoint).  Same protocol on the oracle; SALI at
+    every checkpoint and the accumulated counts agree, on the tile and on the thread layout."""
+    for side in (12, 68):                      # 144 ICs: 4-lane tile; 4624 ICs: one thread per trajectory
+        y0 = W.hh_grid(0.125, side, side)
+        n_ic = y0.shape[1]
+        w0 = W.deviation_vectors(n_ic, 2, 4, 5, "unit")
+        if side == 68:                         # oracle on a sample of the large ensemble
+            idx = np.random.default_rng(2).choice(n_ic, 96, replace=False)
+        else:
+            idx = np.arange(n_ic)
+        yo, wo = np.ascontiguousarray(y0[:, idx]), np.ascontiguousarray(w0[:, :, idx])
+        yg, wg, rep = dev(y0), dev(w0), chs.Report(n_ic, "cuda")
+        cps = [0.0, 40.0, 80.0, 120.0, 160.0]
+        acc_g, acc_o = np.zeros(n_ic, dtype=np.int64), np.zeros(len(idx), dtype=np.int64)
+        for j in range(len(cps) - 1):
+            rep.resume = j > 0
+            sg = chs.sali(HH, None, yg, wg, renorm_every=1, adaptive=True, t0=cps[j], t_end=cps[j + 1], rtol=1e-11,
+                          atol=1e-11, report=rep).cpu().numpy()[0]
+            ro = orc.sali(HH, None, yo, wo, renorm_every=1, adaptive=True, t0=cps[j], t_end=cps[j + 1], rtol=1e-11,
+                          atol=1e-11, precision="f80")
+            so = ro["series"][0]
+            acc_g += rep.n_accepted.cpu().numpy()
+            acc_o += ro["n_accepted"]
+            assert (rep.status.cpu().numpy() == 0).all() and (rep.t_final.cpu().numpy() == cps[j + 1]).all()
+            reg = so > 1e-4
+            assert reg.sum() > 0.5 * len(idx) and np.abs(sg[idx][reg] / so[reg] - 1).max() <= 1e-6
+            assert rel_state(yg.cpu().numpy()[:, idx], yo)[reg].max() <= 1e-8   # (chaotic orbits diverge: R16)
+        assert abs(acc_g[idx].sum() / acc_o.sum() - 1) <= 5e-3
