@@ -193,9 +193,9 @@ __device__ __forceinline__ double logacc_value(const LogAcc& a) {
     return fma((double)a.e, 0.693147180559945309417232, log(a.m));
 }
 
-// Threads per block never exceed this (every launcher uses 64 or 128): size of the per-thread
+// Threads per block never exceed this (every launcher uses 64, 128 or 256): size of the per-thread
 // "cold state" arrays in shared memory.
-constexpr int kMaxTpb = 128;
+constexpr int kMaxTpb = 256;
 
 // NV deferred-log accumulators per thread.  COLD = false: in registers.  COLD = true: in shared memory
 // ([accumulator][thread]: conflict-free), for kernels whose step needs every register -- the accumulators

@@ -84,7 +84,8 @@ int fput_basic_set(const LaunchReq& rq) {
     if (w == WHAT_LD && k == 0 && !ad) return run_chain_ld_t<H, 2, PAD, 128, 4>(rq);
     if (w == WHAT_LD && k == 0 && ad) return run_chain_ld_adapt_t<H, 2, PAD, 128, 2>(rq);
     if (w == WHAT_SALI && k == 2 && !ad) return run_chain_t<H, 2, PAD, 2, MODE_NORM, IND_SALI, false, 128, 2>(rq);
-    if (w == WHAT_GALI && k == 4 && !ad) return run_chain_t<H, 2, PAD, 4, MODE_NORM, IND_GALI, false, 128, 2, true>(rq);
+    // (blocks of 256, one per SM: 440 ms against 445 ms with two blocks of 128 for BASELINE configs[4])
+    if (w == WHAT_GALI && k == 4 && !ad) return run_chain_t<H, 2, PAD, 4, MODE_NORM, IND_GALI, false, 256, 1, true>(rq);
     if constexpr (NS <= 32) {  // one particle per lane: these need more registers per pair
         if (w == WHAT_LYAP && k == 4 && !ad) return run_chain_t<NS, 1, PAD, 4, MODE_MGS, IND_NONE, false, 128, 2>(rq);
         if (w == WHAT_GALI && k == 4 && ad) return run_chain_t<NS, 1, PAD, 4, MODE_NORM, IND_GALI, true, 128, 2>(rq);
