@@ -711,9 +711,16 @@ def main(argv=None):
                 per[name] = measure_config(chs, torch, flush, args, name, dfma_tflops, orc)
             if not args.no_sweeps:
                 out["sweeps"] = run_sweeps(chs, torch, flush, args)
+                # the widened rows of SURVEY 8(f), driver-timed in the same line: f-2 LD of neighbouring ICs and
+                # the adaptive LD on the C2 grid, f-3 the double pendulum (Fig. 1 shape)
+                a3 = argparse.Namespace(**vars(args))
+                a3.config_steps = 2
+                out["widened"] = {n: measure_config(chs, torch, flush, a3, n, dfma_tflops, None)
+                                  for n in ("LDN", "LDA", "F1")}
         out["per_config"] = per
         out["per_config_clocks"] = cs2.summary()
-        out["gpu_launches_total"] = out["gpu_launches"] + sum(2 + args.config_steps + 4 for n in names if n != "C2")
+        out["gpu_launches_total"] = (out["gpu_launches"] + sum(2 + args.config_steps + 4 for n in names if n != "C2")
+                                     + (0 if args.no_sweeps else 3 * (2 + 2 + 4)))
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
