@@ -151,8 +151,7 @@ int chaoticus_ld(const chs_problem* pb, long long n_ic, const double* y0, double
  *  y0            DEVICE [n][n_ic], NOT modified;  ld_fwd, ld_bwd DEVICE [n_ic], either may be NULL
  *  rep           optional; its arrays are [2][n_ic] here (row 0 forward, row 1 backward; the row of a direction
  *                that was not asked for is left untouched); carry / resume are ignored.
- * A trajectory that does not end with status 0 gets NaN.  Separable systems only (the double pendulum
- * returns CHS_EUNSUPPORTED). */
+ * A trajectory that does not end with status 0 gets NaN. */
 int chaoticus_ld_adaptive(const chs_problem* pb, long long n_ic, const double* y0, const chs_stepper* st,
                           double* ld_fwd, double* ld_bwd, const chs_report* rep, void* stream);
 

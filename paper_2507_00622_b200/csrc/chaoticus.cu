@@ -439,7 +439,7 @@ static int ld_adaptive_common(const chs_problem* pb, long long n_ic, const doubl
     }
     if (n_ic == 0 && !info) return CHS_OK;
     QueueLease lease;
-    if (!info && g_adaptive_refill.load() != 0) {
+    if (!info && g_adaptive_refill.load() != 0 && pb->system != CHS_SYS_DOUBLE_PENDULUM) {
         lease = acquire_queue(rq.stream);
         a.queue = lease.counter;
     }

@@ -441,10 +441,11 @@ struct Col {
 };
 
 // Starting step of the adaptive solver (item 6), any layout S
-template <class S>
+// LD: the state carries one more component M (M = 0, M' = |f|_2, scale = atol): run_kernel's LD runs
+template <class S, bool LD = false>
 __device__ __forceinline__ double initial_step(const S& s, double interval, double dir, double rtol, double atol) {
     constexpr int NI = S::NI, L = S::L;
-    const double D = s.dcount();
+    const double D = s.dcount() + (LD ? 1.0 : 0.0);
     if (interval == 0.0) return 0.0;
     bool on[NI];
     s.on_mask(on);
@@ -459,7 +460,18 @@ __device__ __forceinline__ double initial_step(const S& s, double interval, doub
             s1 += (s.p[c] * iq) * (s.p[c] * iq) + (F0[c] * ip) * (F0[c] * ip);
         }
     }
-    const double d0 = sqrt(tile_sum<L>(s0) / D), d1 = sqrt(tile_sum<L>(s1) / D);
+    double nf0 = 0.0;  // LD: |f(y)|_2 = |(p, F0)|_2
+    if constexpr (LD) {
+        double n2 = 0.0;
+#pragma unroll
+        for (int c = 0; c < NI; c++)
+            if (on[c]) n2 = fma(s.p[c], s.p[c], fma(F0[c], F0[c], n2));
+        nf0 = sqrt(tile_sum<L>(n2));
+    }
+    s0 = tile_sum<L>(s0);
+    s1 = tile_sum<L>(s1);
+    if constexpr (LD) s1 += (nf0 / atol) * (nf0 / atol);
+    const double d0 = sqrt(s0 / D), d1 = sqrt(s1 / D);
     double ha = (d0 < 1e-5 || d1 < 1e-5) ? 1e-6 : 0.01 * d0 / d1;
     ha = fmin(ha, interval);
 #pragma unroll
@@ -475,7 +487,16 @@ __device__ __forceinline__ double initial_step(const S& s, double interval, doub
         const double dq = (p1[c] - s.p[c]) * iq, dp = (F1[c] - F0[c]) * ip;
         if (on[c]) s2 += dq * dq + dp * dp;
     }
-    const double d2 = sqrt(tile_sum<L>(s2) / D) / ha;
+    s2 = tile_sum<L>(s2);
+    if constexpr (LD) {
+        double n2 = 0.0;
+#pragma unroll
+        for (int c = 0; c < NI; c++)
+            if (on[c]) n2 = fma(p1[c], p1[c], fma(F1[c], F1[c], n2));
+        const double dn = (sqrt(tile_sum<L>(n2)) - nf0) / atol;
+        s2 += dn * dn;
+    }
+    const double d2 = sqrt(s2 / D) / ha;
     double hb;
     if (d1 <= 1e-15 && d2 <= 1e-15) hb = fmax(1e-6, 1e-3 * ha);
     else hb = root8(0.01 / fmax(d1, d2));
@@ -781,7 +802,7 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
                     for (int c = 0; c < NC; c++) qc[c] = pc[c] = 0.0;
                 }
                 s.template do_renorm<MODE>(false, got && !a.resume);  // on entry: no log accumulated
-                const double h_init = a.h0 > 0.0 ? a.h0 : initial_step(s, interval, dir, a.rtol, a.atol);
+                const double h_init = a.h0 > 0.0 ? a.h0 : initial_step<C, LD>(s, interval, dir, a.rtol, a.atol);
                 if (got) h_abs = h_init;
                 need = false;
                 if (!group_any<L>(!done)) break;

@@ -130,17 +130,30 @@ __device__ __forceinline__ void dop8_generic_stages(const Tab& tab, const typena
     });
 }
 
-template <class Sys, bool ADAPT, int TPB, int MINB>
+// LD (adaptive only): the arc-length Lagrangian descriptor as one more component of the state (R21,
+// as run_kernel's LD): threads are (direction, IC) tasks, the backward pass is the forward pass of (theta, -p);
+// only M and the report ([2][n_ic]) are written.
+template <class Sys, bool ADAPT, int TPB, int MINB, bool LD = false>
 __global__ void __launch_bounds__(TPB, MINB)
 gen_run_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, const RunArgs a) {
+    static_assert(!LD || ADAPT, "LD rides on the adaptive run");
     constexpr int N = Sys::N;
-    const long long ic = (long long)blockIdx.x * TPB + threadIdx.x;
-    if (ic >= a.n_ic) return;
+    const long long task = (long long)blockIdx.x * TPB + threadIdx.x;
+    if (task >= (LD ? a.n_ic * a.n_dirs : a.n_ic)) return;
+    const long long ic = LD ? task % a.n_ic : task;
+    const int dsel = LD ? a.dir_first + (int)(task / a.n_ic) : 0;
+    const long long out_slot = (long long)dsel * a.n_ic + ic;
+    double M = 0.0;
     double y[N], yc[N];  // state and the carried rounding word of its compensated update
 #pragma unroll
     for (int c = 0; c < N; c++) {
-        y[c] = a.y[(long long)c * a.n_ic + ic];
-        yc[c] = (a.resume && a.carry) ? a.carry[(long long)c * a.n_ic + ic] : 0.0;
+        if constexpr (LD) {
+            y[c] = a.y0[(long long)c * a.n_ic + ic] * ((c >= N / 2 && dsel == 1) ? -1.0 : 1.0);
+            yc[c] = 0.0;
+        } else {
+            y[c] = a.y[(long long)c * a.n_ic + ic];
+            yc[c] = (a.resume && a.carry) ? a.carry[(long long)c * a.n_ic + ic] : 0.0;
+        }
     }
     long long n_acc = 0, n_rej = 0;
     int status = ST_OK;
@@ -194,19 +207,34 @@ gen_run_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, 
                     s0 += (y[c] * is) * (y[c] * is);
                     s1 += (f0[c] * is) * (f0[c] * is);
                 }
-                const double d0 = sqrt(s0 / N), d1 = sqrt(s1 / N);
+                constexpr double DD = N + (LD ? 1 : 0);  // LD: one more component M (M = 0, M' = |f|, scale atol)
+                double nf0 = 0.0;
+                if constexpr (LD) {
+#pragma unroll
+                    for (int c = 0; c < N; c++) nf0 = fma(f0[c], f0[c], nf0);
+                    nf0 = sqrt(nf0);
+                    s1 += (nf0 / a.atol) * (nf0 / a.atol);
+                }
+                const double d0 = sqrt(s0 / DD), d1 = sqrt(s1 / DD);
                 double ha = (d0 < 1e-5 || d1 < 1e-5) ? 1e-6 : 0.01 * d0 / d1;
                 ha = fmin(ha, interval);
 #pragma unroll
                 for (int c = 0; c < N; c++) y1[c] = fma(ha * dir, f0[c], y[c]);
                 Sys::rhs(prm, y1, f1);
+                if constexpr (LD) {
+                    double nf1 = 0.0;
+#pragma unroll
+                    for (int c = 0; c < N; c++) nf1 = fma(f1[c], f1[c], nf1);
+                    const double dn = (sqrt(nf1) - nf0) / a.atol;
+                    s2 += dn * dn;
+                }
 #pragma unroll
                 for (int c = 0; c < N; c++) {
                     const double is = 1.0 / fma(fabs(y[c]), a.rtol, a.atol);
                     const double d = (f1[c] - f0[c]) * is;
                     s2 += d * d;
                 }
-                const double d2 = sqrt(s2 / N) / ha;
+                const double d2 = sqrt(s2 / DD) / ha;
                 const double hb = (d1 <= 1e-15 && d2 <= 1e-15) ? fmax(1e-6, 1e-3 * ha) : root8(0.01 / fmax(d1, d2));
                 h_abs = fmin(fmin(100.0 * ha, hb), interval);
             }
@@ -229,6 +257,28 @@ gen_run_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, 
             dop8_generic_stages<Sys, false>(tab, prm, h, y, K);
             double inc[N], yn[N], ycn[N];
             double S5 = 0.0, S3 = 0.0;
+            double Mn = 0.0;
+            if constexpr (LD) {  // M+ = M + |h| sum b_i |K_i|_2 and the embedded errors of M (divided by h)
+                double sb = 0.0, s5 = 0.0, s3 = 0.0;
+                static_for<0, 12>([&](auto lc) {
+                    constexpr int l = decltype(lc)::value;
+                    if constexpr (coef::B[l] != 0.0) {
+                        double n2 = 0.0;
+#pragma unroll
+                        for (int c = 0; c < N; c++) n2 = fma(K[l][c], K[l][c], n2);
+                        const double nr = fast_sqrt(n2);
+                        sb = fma(tab.bl[l], nr, sb);
+                        s5 = fma(tab.e5p[l], nr, s5);
+                        s3 = fma(tab.e3p[l], nr, s3);
+                    }
+                });
+                Mn = fma(h_try, sb, M);
+                const double isc = fast_rcp(fma(a.rtol, fmax(fabs(M), fabs(Mn)), a.atol));
+                s5 *= isc;
+                s3 *= isc;
+                S5 = s5 * s5;
+                S3 = s3 * s3;
+            }
 #pragma unroll
             for (int c = 0; c < N; c++) {
                 double s = tab.bp[0] * K[0][c], e5 = tab.e5p[0] * K[0][c], e3 = tab.e3p[0] * K[0][c];
@@ -250,10 +300,11 @@ gen_run_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, 
                 S5 = fma(u, u, S5);
                 S3 = fma(v, v, S3);
             }
-            const StepDecision dec = step_decision(h_try, S5, S3, (double)N, rejected);
+            const StepDecision dec = step_decision(h_try, S5, S3, (double)(N + (LD ? 1 : 0)), rejected);
             if (dec.acc) {
                 h_abs = h_try * dec.factor;
                 t = t_new;
+                if constexpr (LD) M = Mn;
                 bool fin = true;
 #pragma unroll
                 for (int c = 0; c < N; c++) {
@@ -276,7 +327,17 @@ gen_run_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, 
     bool bad = status != ST_OK;
 #pragma unroll
     for (int c = 0; c < N; c++) bad = bad || !isfinite(y[c]);
+    if constexpr (LD) bad = bad || !isfinite(M);
     if (bad && status == ST_OK) status = ST_NONFINITE;
+    if constexpr (LD) {
+        double* out = dsel == 0 ? a.ld_fwd : a.ld_bwd;
+        out[ic] = bad ? nan("") : M;
+        if (a.n_acc) a.n_acc[out_slot] = n_acc;
+        if (a.n_rej) a.n_rej[out_slot] = n_rej;
+        if (a.status) a.status[out_slot] = status;
+        if (a.t_final) a.t_final[out_slot] = t;
+        return;
+    }
 #pragma unroll
     for (int c = 0; c < N; c++) a.y[(long long)c * a.n_ic + ic] = bad ? nan("") : y[c];
     if (a.carry) {

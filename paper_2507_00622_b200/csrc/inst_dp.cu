@@ -18,6 +18,19 @@ int run_gen(const LaunchReq& rq) {
     return (int)cudaGetLastError();
 }
 template <class Sys, int TPB, int MINB>
+int run_gen_ld_adapt(const LaunchReq& rq) {
+    typename Sys::Params prm;
+    if (!Sys::make_params(rq.params, rq.n_params, prm)) return (int)cudaErrorInvalidValue;
+    auto kern = gen_run_kernel<Sys, true, TPB, MINB, true>;
+    const long long n_threads = rq.args.n_ic * rq.args.n_dirs;
+    int r = finish_launch(rq, kern, TPB, 1, n_threads);
+    if (r != -2) return r;
+    const long long blocks = (n_threads + TPB - 1) / TPB;
+    if (blocks == 0) return 0;
+    kern<<<(unsigned)blocks, TPB, 0, rq.stream>>>(rq.tab, prm, rq.args);
+    return (int)cudaGetLastError();
+}
+template <class Sys, int TPB, int MINB>
 int run_gen_ld(const LaunchReq& rq) {
     typename Sys::Params prm;
     if (!Sys::make_params(rq.params, rq.n_params, prm)) return (int)cudaErrorInvalidValue;
@@ -49,6 +62,7 @@ int try_launch_dp(const LaunchReq& rq) {
     if (CHS_MATCH(3, WHAT_INTEGRATE, 0, 0)) return run_gen<DoublePendulum, false, 128, 3>(rq);
     if (CHS_MATCH(3, WHAT_INTEGRATE, 0, 1)) return run_gen<DoublePendulum, true, 128, 3>(rq);
     if (CHS_MATCH(3, WHAT_LD, 0, 0)) return run_gen_ld<DoublePendulum, 128, 3>(rq);
+    if (CHS_MATCH(3, WHAT_LD, 0, 1)) return run_gen_ld_adapt<DoublePendulum, 128, 3>(rq);
     // solvers 3-6 of PAPER.md:49-52 for the paper's first example system
     if (CHS_MATCH(3, WHAT_SALI, 2, 0)) return run_gen_col<DoublePendulum, 2, 4, MODE_NORM, IND_SALI, false, 128, 3>(rq);
     if (CHS_MATCH(3, WHAT_SALI, 2, 1)) return run_gen_col<DoublePendulum, 2, 4, MODE_NORM, IND_SALI, true, 128, 2>(rq);

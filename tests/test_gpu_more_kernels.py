@@ -573,7 +573,7 @@ def test_fput_spectrum_column_blocks(chs, orc, N, k):
 
 
 # ------------------------------------------------------------------ adaptive Lagrangian descriptor (R21)
-@pytest.mark.parametrize("case", ["hh", "coupled3", "fput8", "fput12_padded", "fput100_wide"])
+@pytest.mark.parametrize("case", ["hh", "coupled3", "fput8", "fput12_padded", "fput100_wide", "double_pendulum"])
 def test_ld_adaptive(chs, orc, case):
     """chaoticus_ld_adaptive (augmented ODE (y, M), M' = |f|, M in the error norm) against the oracle's
     orc_ld_adaptive: two solutions to the same tolerance (R16), so values agree to 1e-8 relative and the
@@ -583,6 +583,8 @@ def test_ld_adaptive(chs, orc, case):
     elif case == "coupled3":
         cfg = W.config("C4", n_ic=333)
         sysid, prm, y0, tau = C3, cfg["params"], cfg["y"], 40.0
+    elif case == "double_pendulum":          # generic first-order kernel
+        sysid, prm, y0, tau = W.SYS_DOUBLE_PENDULUM, (0.5, 2.0), W.double_pendulum_ics(203, seed=11, theta_max=1.0), 25.0
     else:
         N = {"fput8": 8, "fput12_padded": 12, "fput100_wide": 100}[case]
         n_ic = 37 if N == 100 else 301
@@ -642,9 +644,6 @@ def test_ld_adaptive_closed_form_status_and_host(chs):
         chs.ld_adaptive(C3, P, yg, 0.0, -1.0, rtol=1e-9, atol=1e-9)          # tau < 0
     with pytest.raises(chs.ChaoticusError):
         chs.ld_adaptive(C3, P, yg, 0.0, 1.0, rtol=0.0, atol=1e-9)
-    with pytest.raises(chs.ChaoticusError):                                    # not separable: no kernel
-        chs.ld_adaptive(W.SYS_DOUBLE_PENDULUM, (1.0, 1.0), dev(W.double_pendulum_ics(8, seed=1)), 0.0, 1.0,
-                        rtol=1e-9, atol=1e-9)
     assert chs.kernel_info(HH, None, chs.WHAT_LD, adaptive=True, n_ic=1000)["spill_bytes"] == 0
 
 
