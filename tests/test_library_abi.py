@@ -160,16 +160,16 @@ def test_every_kernel_is_spill_free(lib):
     import subprocess
     sass = subprocess.run(["cuobjdump", "-sass", build.LIB], capture_output=True, text=True).stdout
     assert len(sass) > 1_000_000
-    # no local-memory instruction in any kernel, except the double pendulum's: the slow path of the
-    # CUDA library's sincos() (Payne-Hanek reduction of huge arguments) keeps a 40-byte array on the
-    # stack -- library code, not a register spill (ptxas: 0 bytes spill for those kernels too)
+    # no local-memory instruction in ANY kernel (the double pendulum's kernels use fast_sincos, not the CUDA
+    # library's sincos(), whose huge-argument slow path keeps an array on the stack), and no stack frame
     funcs = re.split(r"\n\s*Function : ", sass)
-    assert len(funcs) >= 80
+    assert len(funcs) >= 160
     for f in funcs[1:]:
         name = f.split("\n", 1)[0]
-        if "DoublePendulum" in name:
-            continue
         assert not re.search(r"\b(STL|LDL)\b", f), name
+    logs = "".join(open(os.path.join(build.BUILD, f"ptxas_{u}.log")).read() for u in build.UNITS)
+    frames = re.findall(r"(\d+) bytes stack frame", logs)
+    assert len(frames) >= 160 and all(int(x) == 0 for x in frames)
     assert "DFMA" in sass and "SHFL" in sass
 
 
