@@ -63,7 +63,7 @@ struct DoublePendulum {
         const double x = fma(c1, c2, s1 * s2);   // cos(theta1 - theta2)
         const double sd = fma(s1, c2, -c1 * s2); // sin(theta1 - theta2)
         const double p1 = y[2], p2 = y[3];
-        const double id = 1.0 / fma(-x, x, P.sg1);
+        const double id = fast_rcp(fma(-x, x, P.sg1));  // 1/D, D = 1 + sigma - x^2 > 0; <= 2 ulp, no slow path
         const double m01 = -x * P.ia;
         f[0] = id * fma(P.ia2, p1, m01 * p2);
         f[1] = id * fma(m01, p1, P.sg1 * p2);
@@ -94,7 +94,7 @@ struct DoublePendulum {
         fast_sincos(y[1], &s2, &c2);
         const double x = fma(c1, c2, s1 * s2), sd = fma(s1, c2, -c1 * s2);
         const double p1 = y[2], p2 = y[3];
-        const double id = 1.0 / fma(-x, x, P.sg1), id2 = id * id;
+        const double id = fast_rcp(fma(-x, x, P.sg1)), id2 = id * id;
         const double m01 = -x * P.ia;
         const double Mp0 = fma(P.ia2, p1, m01 * p2), Mp1 = fma(m01, p1, P.sg1 * p2);  // M p
         const double pMp = fma(p1, Mp0, p2 * Mp1), pM1p = -2.0 * P.ia * p1 * p2;           // p^T M p, p^T M' p
