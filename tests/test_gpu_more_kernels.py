@@ -717,3 +717,28 @@ def test_adaptive_indicator_time_series_by_continuation(chs, orc):
             assert reg.sum() > 0.5 * len(idx) and np.abs(sg[idx][reg] / so[reg] - 1).max() <= 1e-6
             assert rel_state(yg.cpu().numpy()[:, idx], yo)[reg].max() <= 1e-8   # (chaotic orbits diverge: R16)
         assert abs(acc_g[idx].sum() / acc_o.sum() - 1) <= 5e-3
+
+
+def test_adaptive_controller_clipping_matches_the_oracle(chs, orc):
+    """The clipping range of the step-size factor (the kernels evaluate 0.9 err^(-1/8) in single precision
+    from num^2 and den, the oracle with pow): err = 0 at an equilibrium -> factor 10 every step (same few
+    accepted steps, none rejected); a hopeless first step h0 = 50 -> rejections with the factor clipped at
+    0.2 until the step fits (same number of rejections); a tiny h0 -> growth by the cap 10 per step."""
+    y0 = W.hh_grid(0.125, 5, 5)
+    y0[:, 3] = 0.0                                   # the equilibrium at the origin: f = 0, err = 0
+    for h0, t_end in ((0.0, 300.0), (50.0, 300.0), (1e-9, 5.0)):
+        yo = y0.copy()
+        ro = orc.integrate_adaptive(HH, None, yo, 0.0, t_end, 1e-10, 1e-10, h0=h0, precision="f64")
+        yg, rep = dev(y0), chs.Report(25, "cuda")
+        chs.integrate_adaptive(HH, None, yg, 0.0, t_end, 1e-10, 1e-10, h0=h0, report=rep)
+        na, nr = rep.n_accepted.cpu().numpy(), rep.n_rejected.cpu().numpy()
+        assert (rep.status.cpu().numpy() == 0).all() and (ro["status"] == 0).all()
+        assert na[3] == ro["n_accepted"][3] and nr[3] == ro["n_rejected"][3] == 0 and na[3] <= 12
+        assert (yg.cpu().numpy()[:, 3] == 0).all()
+        assert (np.abs(na - ro["n_accepted"]) <= 2).all()
+        if h0 == 50.0:                               # 50 -> 10 -> 2 -> 0.4 -> (0.08): at least three clipped rejections
+            assert (nr >= 3)[np.arange(25) != 3].all() and (np.abs(nr - ro["n_rejected"]) <= 1).all()
+        if h0 == 1e-9:                               # growth is capped at 10x per accepted step
+            assert (na >= 8)[np.arange(25) != 3].all()
+            ok = np.arange(25) != 3              # (states only here: at t = 300 chaotic orbits have diverged, R16)
+            assert rel_state(yg.cpu().numpy()[:, ok], yo[:, ok]).max() <= 1e-8
