@@ -11,7 +11,7 @@
 //     lane need none.  A lane evaluates the PPL + 1 springs that touch its particles (the spring it
 //     shares with its right neighbour is evaluated by both: one redundant spring per lane instead of
 //     a second, dependent shuffle).  The walls q_0 = q_{N+1} = 0 (Eq.(8)) are the zeros the first /
-//     last lane substitutes for the missing neighbour, so there is no wall branch.
+//     last lane substitutes for the missing neighbour (a factor 0 inside the difference: no branch, no select).
 //   * PPL = 2 halves the shuffles per particle and removes a third of the spring arithmetic
 //     (BASELINE.json configs[4] runs as LT = 4, PPL = 2: DESIGN.md "Layouts").
 //   * PAD: chains whose length is not LT PPL are padded with particles pinned at zero (coordinates
@@ -39,6 +39,13 @@ struct Chain {
     static constexpr int NSLOT = LT * PPL;
     static constexpr int NCOMP = PPL;      // items 0..PPL-1: the orbit coordinates -- compensated update
     static_assert(NB == 1 || L <= 32, "column blocks live in one warp");
+    // How the first / last lane of an in-warp tile gets the wall's zero in place of the missing neighbour: the
+    // shuffled value enters the difference multiplied by the lane constant wl / wr (0 on the wall lane, 1
+    // elsewhere), d = Q - wl xl as ONE fused multiply-add in place of the subtraction -- instead of selects after
+    // the shuffles (2 FSEL per value: 20 per force evaluation and column pair, 12 % of the instructions of the
+    // adaptive GALI_4 kernel).  With wl in {0, 1} the result is the subtraction's, bit for bit.  Measured
+    // (DESIGN.md section 6): adaptive GALI_4 N = 8 20.6 -> 18.9 ms, Lyapunov k = 4 58.4 -> 55.3 ms, C5 440 -> 434 ms.
+    static constexpr bool WALL_FMA = (LT <= 32);
     using Params = FputParams;
 
     Params prm;
@@ -47,6 +54,7 @@ struct Chain {
     int blk;  // column block (0 .. NB-1)
     int np;   // real chain length (== NSLOT unless PAD)
     mutable int par;  // wide tiles: which half of the edge buffer the next exchange uses
+    double wl, wr;    // 0 on the first / last lane of the tile (the wall), 1 elsewhere (WALL_FMA)
     double q[NI], p[NI];
     LogBank<NCOL, COLD> lg;  // deferred-log accumulators, v >= 1: identical on all lanes of the sub-tile
 
@@ -57,6 +65,8 @@ struct Chain {
         blk = lt / LT;
         np = PAD ? P.np : NSLOT;
         par = 0;
+        wl = (lp == 0) ? 0.0 : 1.0;
+        wr = (lp == LT - 1) ? 0.0 : 1.0;
         lg.init();
         init_walls();
     }
@@ -155,8 +165,10 @@ struct Chain {
             for (int v = 0; v < NCOL; v++) {
                 xl[v] = __shfl_up_sync(0xffffffffu, Q[v * PPL + PPL - 1], 1, LT);
                 xr[v] = __shfl_down_sync(0xffffffffu, Q[v * PPL], 1, LT);
-                if (first) xl[v] = 0.0;
-                if (last) xr[v] = 0.0;
+                if constexpr (!WALL_FMA) {
+                    if (first) xl[v] = 0.0;
+                    if (last) xr[v] = 0.0;
+                }
             }
         } else {
             // wide tile: every thread posts its first and last particle of each column in shared memory
@@ -220,7 +232,9 @@ struct Chain {
         double g[PPL + 1], ph[PPL + 1];
 #pragma unroll
         for (int s = 0; s <= PPL; s++) {
-            const double d = (s == 0) ? Q[0] - xl[0] : (s == PPL) ? xr[0] - Q[PPL - 1] : Q[s] - Q[s - 1];
+            double d;
+            if constexpr (WALL_FMA) d = (s == 0) ? fma(-wl, xl[0], Q[0]) : (s == PPL) ? fma(wr, xr[0], -Q[PPL - 1]) : Q[s] - Q[s - 1];
+            else d = (s == 0) ? Q[0] - xl[0] : (s == PPL) ? xr[0] - Q[PPL - 1] : Q[s] - Q[s - 1];
             ph[s] = fput_phi(prm, d);
             g[s] = fput_g(prm, d);
         }
@@ -232,7 +246,8 @@ struct Chain {
             double T[PPL + 1];  // T[s] = g_s e_s for the inner springs s = 1..PPL-1
 #pragma unroll
             for (int s = 1; s < PPL; s++) T[s] = g[s] * (X[s] - X[s - 1]);
-            const double e0 = X[0] - xl[v], eP = xr[v] - X[PPL - 1];
+            const double e0 = WALL_FMA ? fma(-wl, xl[v], X[0]) : X[0] - xl[v];
+            const double eP = WALL_FMA ? fma(wr, xr[v], -X[PPL - 1]) : xr[v] - X[PPL - 1];
 #pragma unroll
             for (int j = 0; j < PPL; j++) {
                 double f;

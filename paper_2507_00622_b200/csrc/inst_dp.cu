@@ -62,9 +62,9 @@ int try_launch_dp(const LaunchReq& rq) {
     if (CHS_MATCH(3, WHAT_INTEGRATE, 0, 0)) return run_gen<DoublePendulum, false, 128, 3>(rq);
     if (CHS_MATCH(3, WHAT_INTEGRATE, 0, 1)) return run_gen<DoublePendulum, true, 128, 3>(rq);
     if (CHS_MATCH(3, WHAT_LD, 0, 0)) return run_gen_ld<DoublePendulum, 128, 3>(rq);
-    if (CHS_MATCH(3, WHAT_LD, 0, 1)) return run_gen_ld_adapt<DoublePendulum, 128, 3>(rq);
+    if (CHS_MATCH(3, WHAT_LD, 0, 1)) return run_gen_ld_adapt<DoublePendulum, 128, 2>(rq);
     // solvers 3-6 of PAPER.md:49-52 for the paper's first example system
-    if (CHS_MATCH(3, WHAT_SALI, 2, 0)) return run_gen_col<DoublePendulum, 2, 4, MODE_NORM, IND_SALI, false, 128, 3>(rq);
+    if (CHS_MATCH(3, WHAT_SALI, 2, 0)) return run_gen_col<DoublePendulum, 2, 4, MODE_NORM, IND_SALI, false, 128, 2>(rq);
     if (CHS_MATCH(3, WHAT_SALI, 2, 1)) return run_gen_col<DoublePendulum, 2, 4, MODE_NORM, IND_SALI, true, 128, 2>(rq);
     if (CHS_MATCH(3, WHAT_GALI, 2, 0)) return run_gen_col<DoublePendulum, 2, 4, MODE_NORM, IND_GALI, false, 128, 3>(rq);
     if (CHS_MATCH(3, WHAT_GALI, 3, 0)) return run_gen_col<DoublePendulum, 3, 4, MODE_NORM, IND_GALI, false, 128, 3>(rq);
