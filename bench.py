@@ -37,7 +37,7 @@ sys.path.insert(0, ROOT)
 METRIC = "trajectory RK-steps/sec (FP64, incl. variational eqs)"
 UNIT = "RK-steps/s"
 # algorithmic FP64 flop per RK-step of the formulation that runs
-FLOP_PER_STEP = {"C1": 1216.0, "C2": 640.0, "C1sat": 1216.0, "C3": 1746.0, "C4": 4213.0, "C5": 8492.0, "F3": None,
+FLOP_PER_STEP = {"C1": 1216.0, "C2": 640.0, "C1sat": 1216.0, "C3": 1692.0, "C4": 4213.0, "C5": 8492.0, "F3": None,
                  "F1": None, "LDN": 640.0, "LDA": None}
 WORKLOAD_LABEL = {
     "C1": "C1: Henon-Heiles E=1/8, 32x32 grid (1024 ICs), fixed DOP8 h=0.01, 1e4 steps, SALI renormalised every step",

@@ -118,6 +118,7 @@ chs::Tab make_tab(double h) {
         t.e3q[i] = coef::E3Q[i];
         t.e5p[i] = coef::E5[i];
         t.e3p[i] = coef::E3[i];
+        t.d3[i] = coef::B[i] - coef::E3[i];
     }
     t.h = h;
     return t;

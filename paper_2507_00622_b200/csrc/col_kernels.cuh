@@ -648,7 +648,8 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
                     pc[c] = cold_carry[(NC + c) * kMaxTpb + threadIdx.x];
                 }
             }
-            dop8_solution<NI, C::NCOMP, true>(tab, 0.0, s.q, s.p, s.p, F, qn, pn, qc, pc, qcn, pcn);
+            double spo[NI];  // (adaptive kernels only)
+            dop8_solution<NI, C::NCOMP, true>(tab, 0.0, s.q, s.p, s.p, F, qn, pn, qc, pc, qcn, pcn, spo);
 #pragma unroll
             for (int c = 0; c < NI; c++) {
                 s.q[c] = qn[c];
@@ -844,9 +845,10 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
                 hinv = fwd ? fast_rcp(h_try) : -fast_rcp(h_try);  // (h = 0: inf; nothing is committed)
             }
             double qn[NI], pn[NI];
-            dop8_solution<NI, C::NCOMP, false>(tab, hinv, s.q, s.p, u, F, qn, pn, qc, pc, qcn, pcn);
+            double spo[NI];
+            dop8_solution<NI, C::NCOMP, false>(tab, hinv, s.q, s.p, u, F, qn, pn, qc, pc, qcn, pcn, spo);
             double S5, S3;
-            dop8_error_sums<NI>(tab, hinv, s.q, s.p, qn, pn, F, a.rtol, a.atol, on, S5, S3);
+            dop8_error_sums<NI>(tab, hinv, s.q, s.p, qn, pn, F, spo, a.rtol, a.atol, on, S5, S3);
             {
                 double S[2] = {S5, S3};
                 tile_sum_vec<L, 2>(S);
@@ -948,7 +950,8 @@ ld_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const R
         dop8_stages<NI, false>(tab, s.q, s.p, F, force, hook);
         double qn[NI], pn[NI];
         double z[1] = {0.0}, zn[1];
-        dop8_solution<NI, 0, true>(tab, 0.0, s.q, s.p, s.p, F, qn, pn, z, z, zn, zn);
+        double spo[NI];
+        dop8_solution<NI, 0, true>(tab, 0.0, s.q, s.p, s.p, F, qn, pn, z, z, zn, zn, spo);
 #pragma unroll
         for (int c = 0; c < NI; c++) {
             s.q[c] = qn[c];

@@ -39,6 +39,7 @@ struct Tab {
     double bl[12];      // |h| b         (LD quadrature weights)
     double e5q[12], e3q[12];  // (adaptive, raw) E5^T A, E3^T A
     double e5p[12], e3p[12];  // (adaptive, raw) E5, E3
+    double d3[12];            // (adaptive, raw) b - E3: non-zero at stages 1, 9 and 12 only
     double h;                 // signed step (fixed) or 1
 };
 
@@ -317,7 +318,8 @@ __device__ __forceinline__ void dop8_solution(const Tab& tab, double hinv, const
                                               const double (&qc)[NCOMP > 0 ? NCOMP : 1],
                                               const double (&pc)[NCOMP > 0 ? NCOMP : 1],
                                               double (&qcn)[NCOMP > 0 ? NCOMP : 1],
-                                              double (&pcn)[NCOMP > 0 ? NCOMP : 1]) {
+                                              double (&pcn)[NCOMP > 0 ? NCOMP : 1], double (&spo)[NI]) {
+    // spo (adaptive): sum_l b_l G_l per item, which the third-order error estimate reuses (dop8_error_sums)
 #pragma unroll
     for (int c = 0; c < NI; c++) {
         const bool comp = c < NCOMP;
@@ -339,6 +341,7 @@ __device__ __forceinline__ void dop8_solution(const Tab& tab, double hinv, const
                 if constexpr (l > 0 && coef::B[l] != 0.0) sp = fma(tab.bp[l], F[l][c], sp);
             });
             ap = comp ? fma(hinv, sp, pc[comp ? c : 0]) : fma(hinv, sp, p[c]);
+            spo[c] = sp;
         }
         if (comp) {  // aq, ap are increments (+ carried error): Fast2Sum
             const double tq = q[c] + aq, tp = p[c] + ap;
@@ -362,8 +365,8 @@ template <int NI>
 __device__ __forceinline__ void dop8_error_sums(const Tab& tab, double hinv, const double (&q)[NI],
                                                 const double (&p)[NI], const double (&qn)[NI],
                                                 const double (&pn)[NI], const double (&F)[12][NI],
-                                                double rtol, double atol, const bool (&on)[NI], double& S5,
-                                                double& S3) {
+                                                const double (&sp)[NI], double rtol, double atol,
+                                                const bool (&on)[NI], double& S5, double& S3) {
     const double hinv2 = hinv * hinv;
     // NACC interleaved partial sums (items c, c + NACC, ... go to sum c % NACC): the dependent chain is
     // 2 NI / NACC fused multiply-adds deep instead of 2 NI (the error norm is on the serial tail of an attempt)
@@ -372,13 +375,19 @@ __device__ __forceinline__ void dop8_error_sums(const Tab& tab, double hinv, con
 #pragma unroll
     for (int c = 0; c < NI; c++) {
         double s5q = tab.e5q[0] * F[0][c], s3q = tab.e3q[0] * F[0][c];
-        double s5p = tab.e5p[0] * F[0][c], s3p = tab.e3p[0] * F[0][c];
+        double s5p = tab.e5p[0] * F[0][c];
+        // E3 is b with three entries changed (the third-order weights differ from b at stages 1, 9, 12 only):
+        // sum E3_l G_l = sum b_l G_l - sum (b - E3)_l G_l, the first sum being the solution's (3 FMAs, not 8)
+        double s3p = sp[c];
+        static_for<0, 12>([&](auto lc) {
+            constexpr int l = decltype(lc)::value;
+            if constexpr (coef::B[l] != coef::E3[l]) s3p = fma(-tab.d3[l], F[l][c], s3p);
+        });
         static_for<1, 12>([&](auto lc) {
             constexpr int l = decltype(lc)::value;
             if constexpr (coef::E5Q[l] != 0.0) s5q = fma(tab.e5q[l], F[l][c], s5q);
             if constexpr (coef::E3Q[l] != 0.0) s3q = fma(tab.e3q[l], F[l][c], s3q);
             if constexpr (coef::E5[l] != 0.0) s5p = fma(tab.e5p[l], F[l][c], s5p);
-            if constexpr (coef::E3[l] != 0.0) s3p = fma(tab.e3p[l], F[l][c], s3p);
         });
         const double iq = hinv * fast_rcp(fma(rtol, fmax(fabs(q[c]), fabs(qn[c])), atol));
         const double ip = hinv2 * fast_rcp(fma(rtol, fmax(fabs(p[c]), fabs(pn[c])), atol));
