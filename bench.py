@@ -540,8 +540,9 @@ def run_sweeps(chs, torch, flush, args):
                   "linear trend" in the number of degrees of freedom; N spans every tile class (exact and
                   padded in-warp tiles, wide tiles);
     ensemble_size PAPER.md:94, 125 (Fig. 2): the fixed-step SALI kernel, time per IC against the number of
-                  simultaneously integrated ICs."""
-    out = {"fput_dof": [], "ensemble_size": []}
+                  simultaneously integrated ICs;
+    ensemble_size_adaptive  the same curve with the adaptive solver (the solver of the paper's Fig. 2)."""
+    out = {"fput_dof": [], "ensemble_size": [], "ensemble_size_adaptive": []}
     for N in (4, 8, 12, 16, 32, 48, 64, 128):
         a2 = argparse.Namespace(**vars(args))
         a2.workload, a2.fput_n, a2.n_ic, a2.shrink, a2.shrink_ic = "F3", N, 65536, 10, 1
@@ -571,6 +572,31 @@ def run_sweeps(chs, torch, flush, args):
                                      "frac_of_fp64_peak": FLOP_PER_STEP["C1sat"] * rk / (med * 1e-3) / 1e12 / NOMINAL_FP64_TFLOPS,
                                      "lanes": wk["kinfo"]["lanes"]})
         del wk
+        torch.cuda.empty_cache()
+    # the same curve with the ADAPTIVE solver (the solver of the paper's Fig. 2): Henon-Heiles E = 1/8, SALI,
+    # rtol = atol = 1e-12, t = 100
+    from paper_2507_00622_b200 import workloads as W
+    for side in (32, 64, 128, 256, 512):
+        y0 = torch.from_numpy(W.hh_grid(0.125, side, side)).cuda()
+        n_ic = y0.shape[1]
+        w0 = torch.from_numpy(W.deviation_vectors(n_ic, 2, 4, 0, "unit")).cuda()
+        yb, wb, rep = torch.empty_like(y0), torch.empty_like(w0), chs.Report(n_ic, "cuda")
+
+        def prepare():
+            yb.copy_(y0)
+            wb.copy_(w0)
+        wk = dict(prepare=prepare, step_dev=lambda: chs.sali(chs.SYS_HENON_HEILES, None, yb, wb, renorm_every=1, adaptive=True,
+                                                             t_end=100.0, rtol=1e-12, atol=1e-12, report=rep))
+        prepare()
+        wk["step_dev"]()
+        ms = timed(torch, flush, wk, 2)
+        med = float(np.median(ms))
+        att = int(rep.n_accepted.sum().item()) + int(rep.n_rejected.sum().item())
+        out["ensemble_size_adaptive"].append({
+            "n_ic": n_ic, "t_end": 100.0, "ms": med, "us_per_ic": 1e3 * med / n_ic, "attempts": att,
+            "attempts_per_s": att / (med * 1e-3),
+            "lanes": chs.kernel_info(chs.SYS_HENON_HEILES, None, chs.WHAT_SALI, k=2, adaptive=True, n_ic=n_ic)["lanes"]})
+        del wk, y0, w0, yb, wb
         torch.cuda.empty_cache()
     return out
 
