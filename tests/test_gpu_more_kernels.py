@@ -742,3 +742,26 @@ def test_adaptive_controller_clipping_matches_the_oracle(chs, orc):
             assert (na >= 8)[np.arange(25) != 3].all()
             ok = np.arange(25) != 3              # (states only here: at t = 300 chaotic orbits have diverged, R16)
             assert rel_state(yg.cpu().numpy()[:, ok], yo[:, ok]).max() <= 1e-8
+
+
+def test_adaptive_calls_in_flight_on_many_streams(chs):
+    """More adaptive calls in flight than the library has work counters (64 per device): every call owns its
+    counter until its kernel has finished, and a call that finds none free runs without lane refill -- same
+    results either way.  96 calls on 96 streams, enqueued back to back, all equal to the single-call result."""
+    import torch
+    y0 = W.hh_grid(1.0 / 6.0, 30, 20)
+    w0 = W.deviation_vectors(600, 2, 4, 3, "unit")
+    yr, wr = dev(y0), dev(w0)
+    ref = chs.sali(HH, None, yr, wr, renorm_every=1, adaptive=True, t_end=120.0, rtol=1e-11, atol=1e-11)
+    torch.cuda.synchronize()
+    streams = [torch.cuda.Stream() for _ in range(96)]
+    ys = [dev(y0) for _ in streams]
+    ws = [dev(w0) for _ in streams]
+    torch.cuda.synchronize()
+    outs = []
+    for st, yg, wg in zip(streams, ys, ws):
+        with torch.cuda.stream(st):
+            outs.append(chs.sali(HH, None, yg, wg, renorm_every=1, adaptive=True, t_end=120.0, rtol=1e-11, atol=1e-11))
+    torch.cuda.synchronize()
+    for o, yg, wg in zip(outs, ys, ws):
+        assert torch.equal(o, ref) and torch.equal(yg, yr) and torch.equal(wg, wr)
