@@ -35,7 +35,7 @@
 extern "C" {
 #endif
 
-#define CHAOTICUS_VERSION 200 /* 0.2.0 */
+#define CHAOTICUS_VERSION 210 /* 0.2.1: + chaoticus_ld_adaptive(_host) */
 
 typedef enum { CHS_OK = 0, CHS_EINVAL = 1, CHS_EUNSUPPORTED = 2, CHS_ECUDA = 3 } chs_rc;
 
