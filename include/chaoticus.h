@@ -35,7 +35,7 @@
 extern "C" {
 #endif
 
-#define CHAOTICUS_VERSION 210 /* 0.2.1: + chaoticus_ld_adaptive(_host) */
+#define CHAOTICUS_VERSION 220 /* 0.2.2: + chaoticus_ld_neighbour_diffs_noalloc */
 
 typedef enum { CHS_OK = 0, CHS_EINVAL = 1, CHS_EUNSUPPORTED = 2, CHS_ECUDA = 3 } chs_rc;
 
@@ -169,6 +169,33 @@ int chaoticus_ld_adaptive(const chs_problem* pb, long long n_ic, const double* y
 int chaoticus_ld_neighbours(const chs_problem* pb, long long n_ic, const double* y0, double sigma, double t0,
                             double h, long long n_steps, double* ld_fwd, double* ld_bwd, double* diff_fwd,
                             double* diff_bwd, void* stream);
+
+/* The differences of chaoticus_ld_neighbours for callers that CANNOT ALLOCATE device memory.
+ * Some programs may launch work but never call cudaMalloc: a code embedded in an application that handed the
+ * whole HBM to its own pool at start-up (an allocation then fails or breaks a memory budget), or a loop with
+ * a latency bound, where the device-wide synchronisation hidden in cudaMalloc / cudaFree stalls all streams.
+ * chaoticus_ld_neighbours makes such a caller own (1 + 2n) n_ic doubles per direction for the members'
+ * descriptors although it may only want the 2n differences; this call keeps the members' descriptors in a
+ * fixed array inside the library instead and hands back the differences alone.
+ *  y0, sigma, t0, h, n_steps   as chaoticus_ld_neighbours (y0 DEVICE [n][n_ic], not modified)
+ *  diff_fwd, diff_bwd          DEVICE [2n][n_ic], either may be NULL (both NULL: no-op): the same values,
+ *                              bit for bit, as chaoticus_ld_neighbours writes to its diff arrays
+ * Limit: the scratch is CHS_NOALLOC_MAX_DOUBLES doubles (8 MiB, resident on every GPU that loads the library
+ * until the process ends).  A call needs round_up((1 + 2n) n_ic, 32) doubles per requested direction --
+ * Henon-Heiles with both directions: n_ic <= 58 254.  A larger request returns CHS_EINVAL with the numbers in
+ * chaoticus_last_error() and launches nothing; split the ensemble into slices (ICs are independent).
+ * The call allocates and frees nothing: no cudaMalloc / cudaFree / cudaMallocAsync, no event or stream is
+ * created.  It only enqueues on `stream`, like the other device-pointer entry points.
+ * First call on a device: the library looks up the array's device address (cudaGetSymbolAddress, which also
+ * makes the driver load the module there).  Make that first call during set-up, outside any stream capture.
+ * Sharing: all calls on a device use the SAME array, and it keeps the previous call's contents.  Nothing in
+ * it needs clearing (a call overwrites every element it later reads), but two calls whose GPU work overlaps --
+ * different streams, or different host threads without ordering between their streams -- race on it and
+ * give garbage.  Order them (one stream, or events) or use chaoticus_ld_neighbours with your own arrays. */
+#define CHS_NOALLOC_MAX_DOUBLES (1 << 20)
+int chaoticus_ld_neighbour_diffs_noalloc(const chs_problem* pb, long long n_ic, const double* y0, double sigma,
+                                         double t0, double h, long long n_steps, double* diff_fwd,
+                                         double* diff_bwd, void* stream);
 
 /* PAPER.md:51-52 (solvers 5, 6): 1 <= k <= n vectors, modified Gram-Schmidt every
  * renorm_every accepted steps and at the end (orthonormalised once on entry),

@@ -26,7 +26,9 @@ EXPORTS = [
     "chaoticus_ld", "chaoticus_ld_adaptive", "chaoticus_ld_neighbours", "chaoticus_lyap", "chaoticus_ld_host",
     "chaoticus_ld_adaptive_host", "chaoticus_ld_neighbours_host", "chaoticus_sali_host", "chaoticus_gali_host",
     "chaoticus_lyap_host", "chaoticus_integrate_host", "chaoticus_kernel_info", "chaoticus_set_option",
+    "chaoticus_ld_neighbour_diffs_noalloc",
 ]
+NOALLOC_MAX_DOUBLES = 1 << 20   # CHS_NOALLOC_MAX_DOUBLES
 
 
 class ChaoticusError(RuntimeError):
@@ -68,6 +70,7 @@ def _load():
     lib.chaoticus_ld_adaptive_host.argtypes = [PP, ll, vp, SP, vp, vp, RP]
     lib.chaoticus_ld_neighbours.argtypes = [PP, ll, vp, dbl, dbl, dbl, ll, vp, vp, vp, vp, vp]
     lib.chaoticus_ld_neighbours_host.argtypes = [PP, ll, vp, dbl, dbl, dbl, ll, vp, vp, vp, vp]
+    lib.chaoticus_ld_neighbour_diffs_noalloc.argtypes = [PP, ll, vp, dbl, dbl, dbl, ll, vp, vp, vp]
     lib.chaoticus_lyap.argtypes = [PP, ll, vp, vp, i, SP, i, vp, vp, RP, vp]
     lib.chaoticus_ld_host.argtypes = [PP, ll, vp, dbl, dbl, ll, vp, vp]
     lib.chaoticus_sali_host.argtypes = [PP, ll, vp, vp, SP, i, i, vp, vp, RP]
@@ -297,6 +300,22 @@ def ld_neighbours(system, params, y0, sigma, t0, h, n_steps, *, forward=True, ba
                                         _dev(df, (2 * n, n_ic), "diff_fwd"), _dev(db, (2 * n, n_ic), "diff_bwd"),
                                         _stream()))
     return dict(fwd=f, bwd=b, diff_fwd=df, diff_bwd=db)
+
+
+def ld_neighbour_diffs_noalloc(system, params, y0, sigma, t0, h, n_steps, diff_fwd=None, diff_bwd=None):
+    """chaoticus_ld_neighbour_diffs_noalloc: the differences |M(x0 +- sigma e_i) - M(x0)| of ld_neighbours for
+    callers that cannot allocate device memory (an embedding application owns all of the HBM, or the loop
+    cannot afford cudaMalloc's device-wide synchronisation).  The caller passes the outputs diff_fwd / diff_bwd
+    (CUDA float64 [2n, n_ic], either may be None) and gets them filled; the members' descriptors stay in a fixed
+    8 MiB array inside the library, so (1 + 2n) * n_ic (rounded up to 32) per direction must fit in
+    NOALLOC_MAX_DOUBLES, else ChaoticusError.  This wrapper allocates nothing either.  All calls share that
+    array: calls whose GPU work overlaps (different streams) race.  Returns None."""
+    pb = _problem(system, params)
+    n = _dim(pb)
+    n_ic = y0.shape[1]
+    _check(_lib.chaoticus_ld_neighbour_diffs_noalloc(
+        C.byref(pb), n_ic, _dev(y0, (n, n_ic), "y0"), sigma, t0, h, int(n_steps),
+        _dev(diff_fwd, (2 * n, n_ic), "diff_fwd"), _dev(diff_bwd, (2 * n, n_ic), "diff_bwd"), _stream()))
 
 
 # ---- host-buffer forms ------------------------------------------------------------------------

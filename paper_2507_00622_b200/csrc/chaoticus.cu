@@ -740,4 +740,94 @@ int chaoticus_integrate_host(const chs_problem* pb, long long n_ic, double* y, c
     return run_host(chs::WHAT_INTEGRATE, pb, n_ic, y, nullptr, 0, st, 1, 0, nullptr, nullptr, nullptr, rep);
 }
 
+// ---- the entry point that allocates nothing ----------------------------------------------------------
+// chaoticus_ld_neighbour_diffs_noalloc (include/chaoticus.h).  Who needs it: code that may launch kernels
+// but must not touch the allocator -- a solver running inside a host application that reserved all of
+// the HBM for its own pool at start-up (cudaMalloc there fails, or steals from a budget someone else
+// audits), or a time-critical loop where the implicit device-wide synchronisation of cudaMalloc / cudaFree
+// would stall every other stream.  Such a caller can own the small outputs (2n differences per IC) but
+// not the (1 + 2n) member descriptors per IC and direction that chaoticus_ld_neighbours wants as arrays;
+// here those intermediate values live in the fixed array below, which belongs to the library image.
+namespace {
+
+// Scratch of the no-alloc entry point: CHS_NOALLOC_MAX_DOUBLES doubles = 8 MiB.  It is part of the
+// loaded module, so every GPU on which this library's kernels are loaded holds these 8 MiB until the
+// process exits.  One array per device, shared by ALL calls; it keeps whatever the last call left.
+static __device__ __align__(256) double g_noalloc_scratch[CHS_NOALLOC_MAX_DOUBLES];
+
+// In HOST code the identifier g_noalloc_scratch is only a handle for the runtime, NOT a device address
+// (handing it to a kernel would fault, or quietly hit host memory on systems where the GPU can reach
+// it).  The usable address is asked for once per device, with that device current, and kept here.
+double* g_noalloc_ptr[kMaxDevices] = {};
+std::mutex g_noalloc_mutex;
+
+cudaError_t noalloc_scratch(double** out) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_ptr[dev]) {
+        double* p = nullptr;
+        e = cudaGetSymbolAddress((void**)&p, g_noalloc_scratch);  // loads the module on `dev` if need be
+        if (e != cudaSuccess) return e;
+        g_noalloc_ptr[dev] = p;
+    }
+    *out = g_noalloc_ptr[dev];
+    return cudaSuccess;
+}
+
+// The difference stencil of ld_diff_kernel, reading the member descriptors straight from the static
+// array (device code of this file may name it; only the host needs the looked-up address):
+// scratch[off + m * n_ic + ic], m < 1 + n_rows  ->  diff[r * n_ic + ic] = |M_{r+1} - M_0|, r < n_rows.
+__global__ void ld_diff_noalloc_kernel(long long off, double* __restrict__ diff, long long n_ic, int n_rows) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_ic * n_rows) return;
+    const double* ld = g_noalloc_scratch + off;
+    diff[i] = fabs(ld[i + n_ic] - ld[i % n_ic]);
+}
+
+}  // namespace
+
+int chaoticus_ld_neighbour_diffs_noalloc(const chs_problem* pb, long long n_ic, const double* y0, double sigma,
+                                         double t0, double h, long long n_steps, double* diff_fwd,
+                                         double* diff_bwd, void* stream) {
+    const int n = dim_of(pb, nullptr);
+    if (n < 0) return fail(CHS_EINVAL, "unknown system or bad params");
+    if (n_ic < 0) return fail(CHS_EINVAL, "n_ic < 0");
+    if (!(sigma >= 0.0) || !std::isfinite(sigma))
+        return fail(CHS_EINVAL, "ld_neighbour_diffs_noalloc: sigma must be finite and >= 0");
+    if (!diff_fwd && !diff_bwd) return CHS_OK;
+    if (n_ic > 0 && !y0) return fail(CHS_EINVAL, "y0 is NULL");
+    // one block of (1 + 2n) n_ic member descriptors per requested direction, each starting on a 256-byte line
+    const long long members = 1 + 2LL * n;
+    const int n_dirs = (diff_fwd ? 1 : 0) + (diff_bwd ? 1 : 0);
+    if (n_ic > (long long)CHS_NOALLOC_MAX_DOUBLES)  // also keeps members * n_ic far from overflow
+        return fail(CHS_EINVAL, "ld_neighbour_diffs_noalloc: n_ic = %lld is beyond the fixed scratch (%lld doubles)", n_ic,
+                    (long long)CHS_NOALLOC_MAX_DOUBLES);
+    const long long block = (members * n_ic + 31) / 32 * 32;
+    if (block * n_dirs > (long long)CHS_NOALLOC_MAX_DOUBLES)
+        return fail(CHS_EINVAL,
+                    "ld_neighbour_diffs_noalloc: %d direction(s) x (1 + 2n = %lld) members x n_ic = %lld needs %lld doubles "
+                    "of scratch, the fixed array holds %lld: split the ensemble or use chaoticus_ld_neighbours",
+                    n_dirs, members, n_ic, block * n_dirs, (long long)CHS_NOALLOC_MAX_DOUBLES);
+    if (n_ic == 0) return CHS_OK;
+    double* scratch = nullptr;
+    const cudaError_t es = noalloc_scratch(&scratch);
+    if (es != cudaSuccess) return fail(CHS_ECUDA, "CUDA error %d: %s", (int)es, cudaGetErrorString(es));
+    const long long off_fwd = 0, off_bwd = diff_fwd ? block : 0;
+    // Nothing in the scratch has to be zero on entry: the LD launch writes every member descriptor of this
+    // call (NaN for a trajectory that blew up) before the stencil, later on the same stream, reads it.
+    const int rc = ld_common(pb, n_ic, y0, t0, h, n_steps, diff_fwd ? scratch + off_fwd : nullptr,
+                             diff_bwd ? scratch + off_bwd : nullptr, stream, nullptr, (int)members, sigma);
+    if (rc != CHS_OK) return rc;
+    const long long total = n_ic * 2LL * n;
+    const unsigned blocks = (unsigned)((total + 255) / 256);
+    if (diff_fwd) ld_diff_noalloc_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(off_fwd, diff_fwd, n_ic, 2 * n);
+    if (diff_bwd) ld_diff_noalloc_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(off_bwd, diff_bwd, n_ic, 2 * n);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(CHS_ECUDA, "CUDA error %d: %s", (int)e, cudaGetErrorString(e));
+    return CHS_OK;
+}
+
 }  // extern "C"

@@ -41,7 +41,7 @@ def test_header_compiles_as_c_and_cxx(tmp_path):
 
 def test_host_logic_without_gpu(lib):
     from paper_2507_00622_b200 import binding as chs
-    assert chs.version() == 210
+    assert chs.version() == 220
     assert chs.dim(chs.SYS_HENON_HEILES) == 4 and chs.dim(chs.SYS_COUPLED3, [1, 2, 3, 0.1]) == 6
     assert chs.dim(chs.SYS_FPUT, [8, 1, 0, 1]) == 16 and chs.dim(chs.SYS_FPUT, [8.5, 1, 0, 1]) == -1
     assert chs.dim(chs.SYS_COUPLED3, [1.0]) == -1 and chs.dim(9) == -1
