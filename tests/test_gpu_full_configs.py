@@ -131,9 +131,20 @@ def test_C4_full(chs, orc):
     T = 1000.0
     den = np.maximum(np.abs(ro["lam"]).max(0), 1.0 / T)
     assert (np.abs(lam[:, idx] - ro["lam"]) / den).max() <= 1e-8
-    lam1 = ro["lam"][0]
+    # States are compared to 1e-10 where round-off is not amplified beyond it, lambda_1 T <= 10.  WHICH sampled
+    # trajectories that leaves out is decided twice, from the oracle's lambda_1 and from the GPU's own, and the
+    # two sets must be the same (a trajectory within 1e-6 of the threshold may fall either way); no flat quota.
+    lam1, lam1_g = ro["lam"][0], lam[0, idx]
     inside = T <= 10.0 / np.maximum(lam1, 10.0 / T)
-    assert inside.sum() > 0.9 * len(idx) and rel_state(yg.cpu().numpy()[:, idx], yo)[inside].max() <= 1e-10
+    inside_g = T <= 10.0 / np.maximum(lam1_g, 10.0 / T)
+    clear = np.abs(lam1 - 10.0 / T) > 1e-6
+    assert (inside == inside_g)[clear].all() and inside.any()
+    ys = yg.cpu().numpy()[:, idx]
+    assert np.isfinite(ys).all() and np.isfinite(yo).all()          # nobody escaped or blew up on either side
+    assert rel_state(ys, yo)[inside].max() <= 1e-10
+    # the left-out (chaotic) ones still follow the oracle as far as e^{lambda_1 T} allows
+    if (~inside).any():
+        assert (rel_state(ys, yo)[~inside] <= 1e-8 * np.exp(lam1[~inside] * T - 10.0)).all()
     # properties at any size: Liouville (sum = 0), pairing, two vanishing exponents
     assert np.abs(lam.sum(0)).max() <= 1e-12
     assert np.abs(lam + lam[::-1]).max() <= 2e-3
