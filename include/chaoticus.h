@@ -98,7 +98,10 @@ typedef struct {
     int* status;           /* [n_ic] CHS_ST_* */
     double* t_final;       /* [n_ic] time reached */
     double* carry;         /* [n][n_ic] (layout of y) in/out: carried rounding words of the orbit
-                              update; written at the end of every run, read on entry iff resume */
+                              update; read on entry iff resume; written at the end of every FIXED-step
+                              run (and of the double pendulum's adaptive integration); the other
+                              adaptive runs carry no words and leave the array as it is (the *_host
+                              forms hand back zeros after such a run with resume = 0) */
     int resume;            /* 0: fresh run (carry starts at 0, w normalised on entry);
                               1: continuation of a previous call (see above) */
 } chs_report;
@@ -206,7 +209,11 @@ int chaoticus_lyap(const chs_problem* pb, long long n_ic, double* y, double* w, 
                    int renorm_every, double* lambda, double* logsum, const chs_report* rep, void* stream);
 
 /* HOST-buffer forms (same meaning; all array arguments HOST, report members HOST or NULL).
- * They allocate device scratch, copy in, run on an internal stream, copy out and synchronise. */
+ * They allocate device scratch, copy in, run on an internal stream, copy out and synchronise.
+ * The scratch comes from a memory pool of the library's own (one per device, stream-ordered allocator);
+ * the device's default pool and its settings are not touched.  The pool keeps what a call frees, so that
+ * the next call does not go to the driver again: chaoticus_set_option("host_pool_trim", bytes_to_keep)
+ * returns the rest.  rep->carry after a fresh (resume = 0) adaptive run is all zeros. */
 int chaoticus_ld_host(const chs_problem* pb, long long n_ic, const double* y0, double t0, double h,
                       long long n_steps, double* ld_fwd, double* ld_bwd);
 int chaoticus_ld_adaptive_host(const chs_problem* pb, long long n_ic, const double* y0, const chs_stepper* st,
@@ -238,7 +245,10 @@ int chaoticus_kernel_info(const chs_problem* pb, int what, int k, int adaptive, 
  * lane runs it: bit-identical outputs on and off).  Neutral on uniform ensembles, faster on ensembles
  * with unequal step counts.  Each call in flight owns one of 64 device work counters per
  * device (tracked by an event recorded after its launch); when all 64 are busy the call is launched
- * without refill instead (same results).  Off: one trajectory per tile, the grid covers the ensemble.  Returns CHS_EINVAL for an unknown name. */
+ * without refill instead (same results).  Off: one trajectory per tile, the grid covers the ensemble.
+ * "host_pool_trim" (value = bytes to keep, >= 0): not a setting but an action -- the memory pool of the
+ * *_host entry points on the current device gives what it holds beyond `value` bytes back to the driver
+ * (it refills on the next *_host call).  Returns CHS_EINVAL for an unknown name. */
 int chaoticus_set_option(const char* name, int value);
 
 const char* chaoticus_last_error(void); /* thread-local, static storage */

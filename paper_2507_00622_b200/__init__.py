@@ -8,8 +8,10 @@ indicators (the hot path of arXiv 2507.00622).
 """
 import importlib
 
-_API = ("integrate_fixed", "integrate_adaptive", "sali", "gali", "ld", "ld_neighbours", "ld_neighbours_host", "ld_neighbour_diffs_noalloc", "lyap", "ld_host", "sali_host", "gali_host",
-        "lyap_host", "integrate_host", "Report", "HostReport", "kernel_info", "dim", "n_samples", "version", "set_option")
+_API = ("integrate_fixed", "integrate_adaptive", "sali", "gali", "ld", "ld_adaptive", "ld_neighbours",
+        "ld_neighbour_diffs_noalloc", "lyap", "ld_host", "ld_adaptive_host", "ld_neighbours_host", "sali_host",
+        "gali_host", "lyap_host", "integrate_host", "Report", "HostReport", "LdReport", "HostLdReport", "kernel_info",
+        "dim", "n_samples", "version", "set_option", "ChaoticusError")
 
 
 def __getattr__(name):

@@ -273,14 +273,31 @@ def ld_adaptive(system, params, y0, t0, tau, *, rtol, atol, h0=0.0, max_steps=0,
     return f, b
 
 
-def ld_adaptive_host(system, params, y0, t0, tau, ld_fwd, ld_bwd, *, rtol, atol, h0=0.0, max_steps=0):
-    """HOST buffers (numpy): y0 [n, n_ic]; ld_fwd / ld_bwd [n_ic] or None, filled in place."""
+class HostLdReport(HostReport):
+    """As LdReport, with host (numpy) arrays [2, n_ic], for ld_adaptive_host."""
+
+    def __init__(self, n_ic):
+        self.n_accepted = np.zeros((2, n_ic), dtype=np.int64)
+        self.n_rejected = np.zeros((2, n_ic), dtype=np.int64)
+        self.status = np.zeros((2, n_ic), dtype=np.int32)
+        self.t_final = np.zeros((2, n_ic))
+        self.carry = None
+        self.resume = False
+
+
+def ld_adaptive_host(system, params, y0, t0, tau, ld_fwd, ld_bwd, *, rtol, atol, h0=0.0, max_steps=0, report=None):
+    """HOST buffers (numpy): y0 [n, n_ic]; ld_fwd / ld_bwd [n_ic] or None, filled in place.
+    report: a HostLdReport (status, step counts and time reached per direction and IC: a trajectory that
+    did not end with status 0 has NaN in ld_fwd / ld_bwd, and the report says why)."""
     pb = _problem(system, params)
     n = _dim(pb)
     n_ic = y0.shape[1]
+    if report is not None and tuple(report.status.shape) != (2, n_ic):
+        raise ValueError(f"report: need a HostLdReport({n_ic}) (arrays [2, n_ic])")
     st = _stepper(adaptive=True, t0=t0, t_end=t0 + tau, rtol=rtol, atol=atol, h0=h0, max_steps=max_steps)
     _check(_lib.chaoticus_ld_adaptive_host(C.byref(pb), n_ic, _host(y0, (n, n_ic), "y0"), C.byref(st),
-                                           _host(ld_fwd, (n_ic,), "ld_fwd"), _host(ld_bwd, (n_ic,), "ld_bwd"), None))
+                                           _host(ld_fwd, (n_ic,), "ld_fwd"), _host(ld_bwd, (n_ic,), "ld_bwd"),
+                                           _rep(report)))
 
 
 def ld_neighbours(system, params, y0, sigma, t0, h, n_steps, *, forward=True, backward=True, diffs=True,

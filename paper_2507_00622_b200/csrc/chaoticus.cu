@@ -99,6 +99,62 @@ int fail(int rc, const char* fmt, ...) {
     return rc;
 }
 
+// Scratch of the host-buffer entry points: one internal stream per host thread, created on first use
+// and destroyed when the thread ends; device buffers come from the stream-ordered allocator, out of a
+// memory pool that belongs to this library (one per device, created on first use, kept for the life of
+// the process).  The pool keeps freed memory (ITS release threshold is unlimited), so after the first call an
+// allocation is a pool look-up, not a cudaMalloc; the device's default pool, which other libraries in the
+// process use, is left as it is.  chaoticus_set_option("host_pool_trim", 0) hands the kept memory back.
+struct HostCtx {
+    cudaStream_t stream = nullptr;
+    int dev = -1;
+    ~HostCtx() {
+        if (stream) cudaStreamDestroy(stream);  // (an error during process teardown is of no consequence)
+    }
+};
+thread_local HostCtx g_host;
+cudaMemPool_t g_host_pool[kMaxDevices] = {};
+std::mutex g_host_pool_mutex;
+
+cudaError_t host_pool(int dev, cudaMemPool_t* out) {
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_host_pool_mutex);
+    if (!g_host_pool[dev]) {
+        cudaMemPoolProps props;
+        std::memset(&props, 0, sizeof props);
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t pool = nullptr;
+        cudaError_t e = cudaMemPoolCreate(&pool, &props);
+        if (e != cudaSuccess) return e;
+        unsigned long long keep = ~0ULL;
+        e = cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        if (e != cudaSuccess) {
+            cudaMemPoolDestroy(pool);
+            return e;
+        }
+        g_host_pool[dev] = pool;
+    }
+    *out = g_host_pool[dev];
+    return cudaSuccess;
+}
+
+// give the memory the current device's pool holds beyond keep_bytes back to the driver
+int trim_host_pool(size_t keep_bytes) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail(CHS_ECUDA, "CUDA error %d: %s", (int)e, cudaGetErrorString(e));
+    if (dev < 0 || dev >= kMaxDevices) return fail(CHS_ECUDA, "device %d out of range", dev);
+    if (g_host.stream && g_host.dev == dev) cudaStreamSynchronize(g_host.stream);  // the frees of this thread's calls
+    std::lock_guard<std::mutex> lock(g_host_pool_mutex);
+    if (!g_host_pool[dev]) return CHS_OK;  // no host-buffer call was made on this device: nothing is held
+    e = cudaMemPoolTrimTo(g_host_pool[dev], keep_bytes);
+    if (e != cudaSuccess) return fail(CHS_ECUDA, "CUDA error %d: %s", (int)e, cudaGetErrorString(e));
+    return CHS_OK;
+}
+
 // coefficients premultiplied by powers of h (fixed step), or raw with h = 1 (adaptive)
 chs::Tab make_tab(double h) {
     using namespace chs;
@@ -295,6 +351,10 @@ int chaoticus_set_option(const char* name, int value) {
     if (name && std::strcmp(name, "adaptive_refill") == 0) {
         g_adaptive_refill.store(value != 0 ? 1 : 0);
         return CHS_OK;
+    }
+    if (name && std::strcmp(name, "host_pool_trim") == 0) {
+        if (value < 0) return fail(CHS_EINVAL, "host_pool_trim: bytes to keep must be >= 0");
+        return trim_host_pool((size_t)value);
     }
     return fail(CHS_EINVAL, "unknown option '%s'", name ? name : "(null)");
 }
@@ -508,16 +568,6 @@ int chaoticus_kernel_info(const chs_problem* pb, int what, int k, int adaptive, 
 
 // ---- host-buffer forms ---------------------------------------------------------------------
 namespace {
-// Scratch of the host-buffer entry points: one internal stream per host thread, created on first use
-// and kept; device buffers come from the stream-ordered allocator (cudaMallocAsync) whose pool keeps
-// freed memory (release threshold = unlimited), so after the first call an allocation is a pool
-// look-up, not a cudaMalloc.
-struct HostCtx {
-    cudaStream_t stream = nullptr;
-    int dev = -1;
-};
-thread_local HostCtx g_host;
-
 cudaError_t host_stream(cudaStream_t* out) {
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
@@ -528,11 +578,6 @@ cudaError_t host_stream(cudaStream_t* out) {
         e = cudaStreamCreateWithFlags(&g_host.stream, cudaStreamNonBlocking);
         if (e != cudaSuccess) return e;
         g_host.dev = dev;
-        cudaMemPool_t pool;
-        if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-            unsigned long long keep = ~0ULL;
-            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-        }
     }
     *out = g_host.stream;
     return cudaSuccess;
@@ -548,7 +593,14 @@ struct DevBuf {
     cudaError_t alloc(size_t b, cudaStream_t stream) {
         bytes = b;
         st = stream;
-        return b ? cudaMallocAsync(&p, b, stream) : cudaSuccess;
+        if (!b) return cudaSuccess;
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) return e;
+        cudaMemPool_t pool = nullptr;
+        e = host_pool(dev, &pool);
+        if (e != cudaSuccess) return e;
+        return cudaMallocFromPoolAsync(&p, b, pool, stream);
     }
 };
 #define CK(x)                                                                                  \
@@ -584,7 +636,12 @@ int run_host(int what, const chs_problem* pb, long long n_ic, double* y, double*
     chs_report drep{nullptr, nullptr, nullptr, nullptr, nullptr, 0};
     if (rep) {
         drep.resume = rep->resume;
-        if (rep->carry) { CK(dcar.alloc(by, stream)); drep.carry = (double*)dcar.p; }
+        if (rep->carry) {
+            CK(dcar.alloc(by, stream));
+            drep.carry = (double*)dcar.p;
+            // a fresh run starts from zero words; the kernels that carry none (adaptive runs) leave them so
+            if (!drep.resume) CK(cudaMemsetAsync(dcar.p, 0, by, stream));
+        }
         if (rep->n_accepted) { CK(dacc.alloc(sizeof(long long) * n_ic, stream)); drep.n_accepted = (long long*)dacc.p; }
         if (rep->n_rejected) { CK(drej.alloc(sizeof(long long) * n_ic, stream)); drep.n_rejected = (long long*)drej.p; }
         if (rep->status) { CK(dstat.alloc(sizeof(int) * n_ic, stream)); drep.status = (int*)dstat.p; }

@@ -640,6 +640,15 @@ def test_ld_adaptive_closed_form_status_and_host(chs):
     fh, bh = np.empty(517), np.empty(517)
     chs.ld_adaptive_host(C3, P, y0, 0.0, 50.0, fh, bh, rtol=1e-12, atol=1e-12)
     assert np.array_equal(fh, f.cpu().numpy()) and np.array_equal(bh, b.cpu().numpy())
+    # the host form hands the report back too: the NaN entries of a run cut short come with their reason
+    hrep = chs.HostLdReport(517)
+    chs.ld_adaptive_host(C3, P, y0, 0.0, 50.0, fh, bh, rtol=1e-12, atol=1e-12, max_steps=25, report=hrep)
+    assert np.isnan(fh).all() and np.isnan(bh).all() and (hrep.status == 3).all()
+    assert np.array_equal(hrep.n_accepted, rep.n_accepted.cpu().numpy())
+    assert np.array_equal(hrep.n_rejected, rep.n_rejected.cpu().numpy())
+    assert np.array_equal(hrep.t_final, rep.t_final.cpu().numpy())
+    with pytest.raises(ValueError):
+        chs.ld_adaptive_host(C3, P, y0, 0.0, 50.0, fh, bh, rtol=1e-12, atol=1e-12, report=chs.HostReport(517))
     with pytest.raises(chs.ChaoticusError):
         chs.ld_adaptive(C3, P, yg, 0.0, -1.0, rtol=1e-9, atol=1e-9)          # tau < 0
     with pytest.raises(chs.ChaoticusError):
@@ -765,3 +774,71 @@ def test_adaptive_calls_in_flight_on_many_streams(chs):
     torch.cuda.synchronize()
     for o, yg, wg in zip(outs, ys, ws):
         assert torch.equal(o, ref) and torch.equal(yg, yr) and torch.equal(wg, wr)
+
+
+# ---------------------------------------------------------------------------- host-buffer forms: carry, pool
+def test_host_adaptive_run_returns_a_clean_carry(chs):
+    """The *_host forms stage rep->carry in device scratch that comes from a pool (recycled memory).  Adaptive
+    runs of the separable systems carry no rounding words and never write that array, so a fresh run must hand
+    back zeros -- not whatever the pool block held -- or a later fixed-step continuation with resume = 1 would
+    add garbage to the orbit.  With resume = 1 the words that went in come back unchanged."""
+    n_ic = 300
+    y0 = np.ascontiguousarray(W.hh_grid(0.125, 20, 15))
+    w0 = W.deviation_vectors(n_ic, 2, 4, 7, "orthonormal")
+    # 1. dirty the pool: a fixed-step host run whose carry block is full of non-zero words, then freed
+    y, w, out, rep = y0.copy(), w0.copy(), np.empty((1, n_ic)), chs.HostReport(n_ic, n=4)
+    chs.sali_host(HH, None, y, w, out, renorm_every=5, h=0.01, n_steps=200, report=rep)
+    assert np.abs(rep.carry).max() > 0.0
+    # 2. fresh adaptive runs with a carry array full of junk on the host side
+    for fn in ("integrate", "sali"):
+        y, w, rep = y0.copy(), w0.copy(), chs.HostReport(n_ic, n=4)
+        rep.carry[:] = 123.0
+        if fn == "integrate":
+            chs.integrate_host(HH, None, y, report=rep, adaptive=True, t0=0.0, t_end=5.0, rtol=1e-10, atol=1e-10)
+        else:
+            chs.sali_host(HH, None, y, w, out, renorm_every=5, report=rep, adaptive=True, t0=0.0, t_end=5.0,
+                          rtol=1e-10, atol=1e-10)
+        assert (rep.status == 0).all() and (rep.carry == 0.0).all(), fn
+        # ... so that a fixed-step continuation from it is the fixed-step run from the same state, bit for bit
+        ya, yb = y.copy(), y.copy()
+        rep.resume = True
+        chs.integrate_host(HH, None, ya, report=rep, h=0.01, n_steps=100)
+        chs.integrate_host(HH, None, yb, h=0.01, n_steps=100)
+        assert np.array_equal(ya, yb), fn
+    # 3. resume = 1 on an adaptive run: the words pass through untouched
+    y, w, rep = y0.copy(), w0.copy(), chs.HostReport(n_ic, n=4)
+    rep.carry[:] = np.random.default_rng(1).normal(size=rep.carry.shape) * 1e-17
+    keep = rep.carry.copy()
+    rep.resume = True
+    chs.sali_host(HH, None, y, w, out, renorm_every=5, report=rep, adaptive=True, t0=0.0, t_end=2.0, rtol=1e-10, atol=1e-10)
+    assert np.array_equal(rep.carry, keep)
+
+
+def test_host_forms_use_their_own_memory_pool(chs):
+    """The scratch of the *_host forms comes from a pool the library owns: the release threshold of the device's
+    DEFAULT pool (which torch's cudaMallocAsync backend or other libraries may use) stays what it was, and
+    set_option("host_pool_trim", 0) gives the memory the library's pool kept back to the driver."""
+    import ctypes
+    import torch
+    rt = ctypes.CDLL("libcudart.so.12")
+    def default_threshold():
+        pool, val = ctypes.c_void_p(), ctypes.c_uint64(12345)
+        assert rt.cudaDeviceGetDefaultMemPool(ctypes.byref(pool), torch.cuda.current_device()) == 0
+        assert rt.cudaMemPoolGetAttribute(pool, 4, ctypes.byref(val)) == 0      # cudaMemPoolAttrReleaseThreshold = 4
+        return val.value
+    before = default_threshold()
+    n_ic = 1 << 20                                           # 32 MiB of states + 16 MiB of outputs
+    y0 = np.ascontiguousarray(np.tile(W.hh_grid(0.125, 4, 4)[:, 5:6], (1, n_ic)))
+    f, b = np.empty(n_ic), np.empty(n_ic)
+    chs.ld_host(HH, None, y0, 0.0, 0.01, 2, f, b)
+    assert default_threshold() == before
+    torch.cuda.synchronize()
+    held = torch.cuda.mem_get_info()[0]
+    chs.set_option("host_pool_trim", 0)
+    freed = torch.cuda.mem_get_info()[0] - held
+    assert freed >= 40 * 2 ** 20, freed                      # the 48 MiB the call used went back
+    f2, b2 = np.empty(n_ic), np.empty(n_ic)
+    chs.ld_host(HH, None, y0, 0.0, 0.01, 2, f2, b2)          # and the pool refills on the next call
+    assert np.array_equal(f, f2) and np.array_equal(b, b2)
+    with pytest.raises(chs.ChaoticusError):
+        chs.set_option("host_pool_trim", -1)

@@ -52,6 +52,21 @@ def test_host_logic_without_gpu(lib):
     assert chs.n_samples(2003, 10, 25) == 201 // 25 + 1
 
 
+def test_package_reexports_the_whole_binding(lib):
+    """Every public function / class of binding.py that wraps an entry point is reachable as
+    paper_2507_00622_b200.<name> (the lazy re-export list once missed ld_adaptive and LdReport)."""
+    import inspect
+    import paper_2507_00622_b200 as pkg
+    from paper_2507_00622_b200 import binding
+    public = [n for n, o in vars(binding).items()
+              if not n.startswith("_") and (inspect.isfunction(o) or inspect.isclass(o)) and o.__module__ == binding.__name__]
+    assert {"ld_adaptive", "ld_adaptive_host", "LdReport", "HostLdReport", "ld_neighbour_diffs_noalloc"} <= set(public)
+    for name in public:
+        assert getattr(pkg, name) is getattr(binding, name), name
+    with pytest.raises(AttributeError):
+        pkg.no_such_entry_point
+
+
 def test_n_samples_matches_oracle(orc):
     from paper_2507_00622_b200 import binding as chs
     for n_steps, m, se in [(0, 1, 1), (1, 1, 1), (999, 10, 3), (1000, 10, 3), (12345, 7, 11)]:
