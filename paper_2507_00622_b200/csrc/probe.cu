@@ -7,6 +7,7 @@
 // mode 2: x_i = fma(x_i, y_i, z_i) with three distinct register operands per DFMA (register-file
 //         bandwidth / bank conflicts included)
 #include <cuda_runtime.h>
+#include "gen_kernels.cuh"  // fast_sincos; brings dop8_core.cuh: fast_sqrt, fast_rsqrt, fast_rcp
 namespace {
 struct PC { double c[16]; };
 template <int MODE>
@@ -43,5 +44,35 @@ extern "C" int chs_probe_dfma(int mode, long long iters, int n_blocks, int n_thr
     if (mode == 0) dfma_probe_kernel<0><<<n_blocks, n_threads, 0, st>>>(iters, out, pc);
     if (mode == 1) dfma_probe_kernel<1><<<n_blocks, n_threads, 0, st>>>(iters, out, pc);
     if (mode == 2) dfma_probe_kernel<2><<<n_blocks, n_threads, 0, st>>>(iters, out, pc);
+    return cudaGetLastError() == cudaSuccess ? 0 : 3;
+}
+
+// ---- the device math helpers, one value per thread (TEST AID: tests/test_gpu_math_helpers.py measures their
+// error against the host's long double; the step kernels inline the same functions) -------------------------
+namespace {
+__global__ void math_probe_kernel(int which, long long n, const double* __restrict__ x, double* __restrict__ o1,
+                                  double* __restrict__ o2) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double v = x[i];
+    if (which == 0) o1[i] = chs::fast_sqrt(v);
+    else if (which == 1) o1[i] = chs::fast_rsqrt(v);
+    else if (which == 2) o1[i] = chs::fast_rcp(v);
+    else {
+        double sn, cs;
+        chs::fast_sincos(v, &sn, &cs);
+        o1[i] = sn;
+        o2[i] = cs;
+    }
+}
+}  // namespace
+// which: 0 fast_sqrt, 1 fast_rsqrt, 2 fast_rcp, 3 fast_sincos (out2 = cos; otherwise out2 is not used).
+// x, out1, out2 DEVICE [n].  Returns 0, 1 (bad argument) or 3 (CUDA error).
+extern "C" int chs_probe_math(int which, long long n, const double* x, double* out1, double* out2, void* stream) {
+    if (which < 0 || which > 3 || n < 0 || (n > 0 && (!x || !out1 || (which == 3 && !out2)))) return 1;
+    if (n == 0) return 0;
+    const long long blocks = (n + 255) / 256;
+    if (blocks > 2147483647LL) return 1;
+    math_probe_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(which, n, x, out1, out2);
     return cudaGetLastError() == cudaSuccess ? 0 : 3;
 }
