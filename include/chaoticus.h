@@ -93,7 +93,10 @@ typedef struct {
 #define CHS_ST_UNDERFLOW 2
 #define CHS_ST_MAXSTEPS 3
 typedef struct {
-    long long* n_accepted; /* [n_ic] accepted steps (fixed: n_steps) */
+    long long* n_accepted; /* [n_ic] accepted steps.  Fixed step: n_steps -- or, for a trajectory whose state
+                              stopped being finite (status CHS_ST_NONFINITE), the step at which it was found
+                              dead: the state is tested after every 8th step and after the last, so this is
+                              at most 7 steps past the step of death; t_final = t0 + n_accepted h */
     long long* n_rejected; /* [n_ic] rejected attempts (fixed: 0) */
     int* status;           /* [n_ic] CHS_ST_* */
     double* t_final;       /* [n_ic] time reached */

@@ -331,6 +331,14 @@ int run_common(int what, const chs_problem* pb, long long n_ic, double* y, doubl
         a.resume = rep->resume ? 1 : 0;
     }
     if (n_ic == 0 && !info) return CHS_OK;
+    // Fixed step: the kernels latch the step at which a trajectory's state first stops being finite in that
+    // trajectory's own report word (n_accepted, else t_final: col_kernels.cuh death_word) by atomicMin, and
+    // rewrite the word with its real content at the end; it starts at all ones = "alive".
+    if (!st->adaptive && !info && (a.n_acc || a.t_final)) {
+        void* word = a.n_acc ? (void*)a.n_acc : (void*)a.t_final;
+        const cudaError_t e = cudaMemsetAsync(word, 0xff, sizeof(long long) * (size_t)n_ic, rq.stream);
+        if (e != cudaSuccess) return fail(CHS_ECUDA, "CUDA error %d: %s", (int)e, cudaGetErrorString(e));
+    }
     QueueLease lease;
     if (st->adaptive && !info && g_adaptive_refill.load() != 0 && pb->system != CHS_SYS_DOUBLE_PENDULUM) {
         lease = acquire_queue(rq.stream);

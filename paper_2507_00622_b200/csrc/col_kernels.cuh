@@ -585,6 +585,29 @@ struct LdNormHook {
     }
 };
 
+// scratch word of a fixed-step trajectory's death step: its n_accepted entry, else its t_final entry (both
+// are 8 bytes and are rewritten with their real content at the end of the run), else none -- then nobody
+// asked where the trajectory died
+__device__ __forceinline__ unsigned long long* death_word(const RunArgs& a, long long ic) {
+    if (a.n_acc) return reinterpret_cast<unsigned long long*>(a.n_acc + ic);
+    if (a.t_final) return reinterpret_cast<unsigned long long*>(a.t_final + ic);
+    return nullptr;
+}
+// non-finite never heals, so the minimum over all notes of a trajectory is the first one
+template <int NI>
+__device__ __forceinline__ void note_death(const RunArgs& a, const double (&q)[NI], const double (&p)[NI], bool valid,
+                                           long long ic, long long st) {
+    if (lane_nonfinite<NI>(q, p)) {  // off the hot path
+        unsigned long long* dw = death_word(a, ic);
+        if (valid && dw) atomicMin(dw, (unsigned long long)st);
+    }
+}
+template <int L>
+__device__ __forceinline__ void tile_sync() {
+    if constexpr (L > 32) __syncthreads();
+    else if constexpr (L > 1) __syncwarp();
+}
+
 // ---- the run kernel: fixed or adaptive, with renormalisation / indicator ----------------------
 // S = the per-lane state class of a layout (Col<Sys,K,L> here, Chain<NP,K> in chain_kernels.cuh)
 // PAIR: evaluate the stages two at a time (dop8_core.cuh dop8_stages); off only where the extra live
@@ -637,7 +660,13 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
                 cold_carry[(NC + c) * kMaxTpb + threadIdx.x] = pc[c];
             }
         }
+        // The step after which the state was first not finite (the oracle tests after every step and stops
+        // there) is latched in GLOBAL memory, in the trajectory's own report word (death_word): the step
+        // kernels have no register to spare for it, and only lanes that are already dead ever touch it.
         for (long long st = 1; st <= a.n_steps; ++st) {
+            // the oracle's test after a step, made on entry to the next one: after every kDeathCheckEvery-th
+            // step here, and after the last one below
+            if (((st - 1) & (kDeathCheckEvery - 1)) == 0 && st > 1) note_death<NI>(a, s.q, s.p, valid, ic, st - 1);
             double F[12][NI];
             dop8_stages<NI, PAIR>(tab, s.q, s.p, F, force, nohook);
             double qn[NI], pn[NI];
@@ -683,12 +712,14 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
                 }
             }
         }
+        if (a.n_steps > 0) note_death<NI>(a, s.q, s.p, valid, ic, a.n_steps);
         n_acc = a.n_steps;
         t = a.t0 + (double)a.n_steps * a.h;
-        const bool bad = !s.finite_all();
-        if (bad) status = ST_NONFINITE;
+        bool bad = !s.finite_all();
         double ind = 0.0;
         if constexpr (IND != IND_NONE) ind = s.template indicator<IND>();
+        if (bad) status = ST_NONFINITE;
+        tile_sync<L>();  // the dead lanes' atomics are ordered before the orbit lane reads the word back
         if (!valid) return;
         s.store(a.y, a.w, a.n_ic, ic, bad);
         if constexpr (COLD) {
@@ -706,6 +737,14 @@ run_kernel(const __grid_constant__ Tab tab, const typename C::Params prm, const 
                     a.series[(a.n_samples - 1) * a.n_ic + ic] = bad ? nan("") : ind;
                     if (bad)
                         for (long long r = slot; r < a.n_samples - 1; r++) a.series[r * a.n_ic + ic] = nan("");
+                }
+            }
+            if (unsigned long long* dw = death_word(a, ic)) {
+                const unsigned long long died = *(volatile unsigned long long*)dw;
+                if (died != ~0ULL) {  // a dead trajectory reports the step at which it died (where the oracle stops)
+                    n_acc = (long long)died;
+                    t = a.t0 + (double)n_acc * a.h;
+                    status = ST_NONFINITE;
                 }
             }
             if (a.n_acc) a.n_acc[ic] = n_acc;

@@ -15,11 +15,16 @@ namespace chs {
 
 // sin and cos of one angle without the CUDA library routine's slow path (its huge-argument reduction keeps a
 // 40-byte stack array -- the only local memory the library had -- behind a branch).  k = rint(x 2/pi);
-// r = x - k pi/2 with pi/2 split into three doubles and fused multiply-adds (the first product is exact and the
-// difference is exactly representable, so r is as accurate as x for every |x| < 2^50); sin r and cos r on
-// [-pi/4, pi/4] by their Taylor polynomials to r^15 / r^16 (remainders 5e-17 r and 2e-18: below half an ulp;
-// the coefficients are (-1)^m / n! rounded to double); the quadrant k mod 4 swaps and negates by selects.
-// 24 FP64 instructions, branch-free.  Measured against sincos() over 4e8 arguments: <= 1 ulp (_work probe).
+// r = x - k pi/2 with pi/2 split into three doubles and three fused multiply-adds.  The first constant is the
+// full 53-bit double nearest pi/2, so k * c1 is NOT a double; what saves the step is the fused multiply-add,
+// which forms x - k c1 from the exact product with ONE rounding (error <= half an ulp of r, about 2^-54 for
+// |r| <= pi/4), and the two corrections add pi/2's next 106 bits times k.  sin r and cos r on [-pi/4, pi/4] by
+// their Taylor polynomials to r^15 / r^16 (remainders 5e-17 r and 2e-18: below half an ulp; the coefficients
+// are (-1)^m / n! rounded to double); the quadrant k mod 4 swaps and negates by selects.  24 FP64
+// instructions, branch-free.  Measured against the host's long double sine and cosine of the same double x
+// over 10^7 arguments, |x| up to 1e8, multiples of pi/2 included (tests/test_gpu_math_helpers.py): <= 2 ulp
+// of the true value everywhere (1.56 seen at |x| = 9.9e6 and 1.54 at |x| <= 10: it is the polynomial's rounding, not
+// the reduction's, that sets it).
 __device__ __forceinline__ void fast_sincos(double x, double* sn, double* cs) {
     const double k = rint(x * 0.6366197723675814);
     double r = fma(-k, 1.5707963267948966, x);
@@ -203,6 +208,7 @@ gen_run_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, 
         yn[c] = s_;                                          \
     }
 
+    long long first_bad = 0;  // fixed step: the first step after which the state was not finite (dop8_core.cuh)
     if constexpr (!ADAPT) {
         for (long long st = 0; st < a.n_steps; ++st) {
             double K[12][N];
@@ -223,9 +229,11 @@ gen_run_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, 
                 y[c] = yn[c];
                 yc[c] = ycn[c];
             }
+            if ((((st + 1) & (kDeathCheckEvery - 1)) == 0 || st + 1 == a.n_steps) && first_bad == 0 && lane_nonfinite<N>(y, y))
+                first_bad = st + 1;
         }
-        n_acc = a.n_steps;
-        t = a.t0 + (double)a.n_steps * a.h;
+        n_acc = first_bad > 0 ? first_bad : a.n_steps;  // a dead trajectory reports the step at which it died
+        t = a.t0 + (double)n_acc * a.h;
     } else {
         const double dir = (a.t_end >= a.t0) ? 1.0 : -1.0;
         const double interval = fabs(a.t_end - a.t0);
@@ -529,6 +537,7 @@ gen_col_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, 
     long long slot = 0;
     if constexpr (!ADAPT) {
         int cd = a.m, sd = a.sample_every;
+        long long first_bad = 0;  // first step after which this lane's column was not finite (dop8_core.cuh)
         for (long long st = 1; st <= a.n_steps; ++st) {
             double Kd[12][N];
             stages(std::true_type{}, 0.0, Kd);
@@ -544,6 +553,8 @@ gen_col_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, 
             }
             advance(inc, yn, ycn);
             commit(yn, ycn);
+            if (((st & (kDeathCheckEvery - 1)) == 0 || st == a.n_steps) && first_bad == 0 && lane_nonfinite<2>(s.q, s.p))
+                first_bad = st;
             if constexpr (MODE != MODE_NONE) {
                 if (--cd == 0 || st == a.n_steps) {
                     cd = a.m;
@@ -562,8 +573,9 @@ gen_col_kernel(const __grid_constant__ Tab tab, const typename Sys::Params prm, 
                 }
             }
         }
-        n_acc = a.n_steps;
-        t = a.t0 + (double)a.n_steps * a.h;
+        const long long died = tile_first_step<L>(first_bad);  // a dead trajectory reports where it died
+        n_acc = died > 0 ? died : a.n_steps;
+        t = a.t0 + (double)n_acc * a.h;
     } else {
         // adaptive: the tile's decisions come from tile-wide sums, identical on
         // all its lanes; tiles of one warp differ, so the loop is warp-uniform and commits are predicated

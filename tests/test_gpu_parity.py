@@ -150,6 +150,105 @@ def test_nonfinite_status(chs):
     assert (st[ok] == 0).all() and np.isfinite(out[:, ok]).all()
 
 
+DEATH_CHECK_EVERY = 8      # csrc/dop8_core.cuh kDeathCheckEvery
+
+
+def _report_matches(rep, ro, t0, h, n_steps):
+    """Report of a fixed-step run against the oracle's.  Live trajectories: identical.  Dead ones: the oracle
+    stops at the step s after which its state is not finite; the kernels test after every 8th step and after
+    the last, so they report the first tested step >= their own s -- and their own s may be s -+ 1: in the
+    step of death magnitudes jump by hundreds of decades and WHICH intermediate overflows first (the kernels
+    carry h^2-scaled forces) decides between two neighbouring steps.  t_final = t0 + n_accepted h on both."""
+    st, na, tf = rep.status.cpu().numpy(), rep.n_accepted.cpu().numpy(), rep.t_final.cpu().numpy()
+    assert np.array_equal(st, ro["status"]), (np.flatnonzero(st != ro["status"]), st[st != ro["status"]])
+    s = ro["n_accepted"]
+    up = lambda x: np.minimum(-(-x // DEATH_CHECK_EVERY) * DEATH_CHECK_EVERY, n_steps)
+    dead = st != 0
+    lo, hi = np.where(dead, up(np.maximum(s - 1, 1)), s), np.where(dead, up(s + 1), s)
+    d = np.flatnonzero((na < lo) | (na > hi))
+    assert d.size == 0, (d, na[d], s[d])
+    assert ((na[dead] % DEATH_CHECK_EVERY == 0) | (na[dead] == n_steps)).all()
+    assert np.abs(tf - (t0 + na * h)).max() <= 4e-16 * np.abs(tf).max()
+    assert np.abs(tf[~dead] - ro["t_final"][~dead]).max(initial=0.0) <= 4e-16 * np.abs(tf).max()
+    assert (rep.n_rejected.cpu().numpy() == 0).all()
+    return st, na
+
+
+@pytest.mark.parametrize("case", ["hh_integrate", "hh_sali_tile", "hh_gali3_thread", "c3_lyap", "fput8_gali4",
+                                  "fput12_gali4_pad", "fput100_sali_wide", "dp_integrate", "dp_sali"])
+def test_fixed_step_dead_trajectories_report_where_they_died(chs, orc, case):
+    """A fixed-step trajectory whose state stops being finite (an escaping orbit: Henon-Heiles above the
+    escape energy, the cubic terms of the 3-DoF system and of the alpha-FPUT chain) is reported as the oracle
+    reports it: status 1, n_accepted = the step after which the state was first found non-finite (tested after
+    every 8th step: _report_matches), t_final = t0 + n_accepted h, outputs NaN -- not the end of the run.  Both sides take that decision in double precision
+    (oracle "f64": the 80-bit oracle overflows later).  Every layout: thread, column tile, chain tile (exact,
+    padded, wide), generic first-order kernels; live neighbours in the same warp are untouched."""
+    rng = np.random.default_rng(11)
+    h, n_steps, m = 0.02, 2000, 7
+    dead = [3, 17, 40]                                       # spread over two warps of the thread layout
+    if case.startswith("hh"):
+        sysid, prm = HH, None
+        y0 = np.ascontiguousarray(W.hh_grid(0.125, 9, 5))     # 45 ICs
+        for j, i in enumerate(dead):
+            y0[:, i] = [0.0, 2.0 + j, 0.0, 3.0 + 2 * j]       # far outside the bounded region: different death steps
+    elif case.startswith("c3"):
+        sysid, prm = C3, W.coupled3_params(0.5)
+        y0 = W.coupled3_ics(45, seed=2, eps=0.5)
+        for j, i in enumerate(dead):
+            y0[:, i] = [3.0 + j, -4.0, -5.0 - j, 0.0, 0.0, 0.0]
+    elif case.startswith("fput"):
+        N = int(case[4:].split("_")[0])
+        sysid, prm = FPUT, W.fput_params(N, 1.0, 1.0, 0.0)    # alpha-FPUT: the cubic potential is unbounded below
+        y0 = W.fput_ics(45, N, seed=4, E=0.01 * N)
+        for j, i in enumerate(dead):
+            y0[:N, i] = -(4.0 + j) * (N + 1) / 9.0 * np.sin(np.pi * np.arange(1, N + 1) / (N + 1))   # same stretch per spring
+    else:
+        sysid, prm = W.SYS_DOUBLE_PENDULUM, (1.0, 1.0)
+        y0 = W.double_pendulum_ics(45, seed=3)
+        y0[2, 3], y0[3, 17], y0[0, 40] = np.inf, -np.inf, np.nan      # the pendulum cannot escape: dead on arrival
+    n, n_ic = y0.shape
+    what = case.split("_")[1]
+    k = {"integrate": 0, "sali": 2, "gali3": 3, "gali4": 4, "lyap": 3}[what]
+    w0 = W.deviation_vectors(n_ic, k, n, 5, "orthonormal") if k else None
+    rep = chs.Report(n_ic, "cuda")
+    yo, yg = y0.copy(), dev(y0)
+    wo, wg = (w0.copy(), dev(w0)) if k else (None, None)
+    if what == "integrate":
+        ro = orc.integrate_fixed(sysid, prm, yo, 0.5, h, n_steps, precision="f64")
+        chs.integrate_fixed(sysid, prm, yg, 0.5, h, n_steps, report=rep)
+    elif what == "sali":
+        ro = orc.sali(sysid, prm, yo, wo, renorm_every=m, sample_every=20, t0=0.5, h=h, n_steps=n_steps, precision="f64")
+        out = chs.sali(sysid, prm, yg, wg, renorm_every=m, sample_every=20, t0=0.5, h=h, n_steps=n_steps, report=rep)
+    elif what.startswith("gali"):
+        ro = orc.gali(sysid, prm, yo, wo, renorm_every=m, sample_every=20, t0=0.5, h=h, n_steps=n_steps, precision="f64")
+        out = chs.gali(sysid, prm, yg, wg, renorm_every=m, sample_every=20, t0=0.5, h=h, n_steps=n_steps, report=rep)
+    else:
+        ro = orc.lyap(sysid, prm, yo, wo, renorm_every=m, t0=0.5, h=h, n_steps=n_steps, precision="f64")
+        out = chs.lyap(sysid, prm, yg, wg, renorm_every=m, t0=0.5, h=h, n_steps=n_steps, report=rep)
+    st, na = _report_matches(rep, ro, 0.5, h, n_steps)
+    assert (st[dead] == chs.ST_NONFINITE).all() and (na[dead] < n_steps).all() and (na[dead] >= 1).all()
+    live = np.delete(np.arange(n_ic), dead)
+    assert (st[live] == 0).all() and (na[live] == n_steps).all()
+    yg = yg.cpu().numpy()
+    assert np.isnan(yg[:, dead]).all() and np.isnan(yo[:, dead]).all() and np.isfinite(yg[:, live]).all()
+    if k:
+        assert np.isnan(wg.cpu().numpy()[:, :, dead]).all() and np.isfinite(wg.cpu().numpy()[:, :, live]).all()
+        out = out.cpu().numpy()
+        ref = ro["lam"] if what == "lyap" else ro["series"]
+        assert np.array_equal(np.isnan(out), np.isnan(ref))   # rows sampled before the death keep their values
+        assert np.isnan(out[-1, dead]).all() and np.isfinite(out[:, live]).all()
+    # a report with t_final only (no n_accepted array) says the same
+    if what == "integrate":
+        import torch
+        rep2 = chs.Report(n_ic, "cuda")
+        c = rep2._struct()
+        c.n_accepted = None
+        rep2._struct = lambda: c
+        y2 = dev(y0)
+        chs.integrate_fixed(sysid, prm, y2, 0.5, h, n_steps, report=rep2)
+        assert torch.equal(rep2.t_final, rep.t_final) and torch.equal(rep2.status, rep.status)
+
+
 # ---------------------------------------------------------------------------- Lagrangian descriptor
 def test_ld_hh(chs, orc):
     y0 = W.hh_grid(0.125, 37, 37)  # 1369 ICs
